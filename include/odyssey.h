@@ -1,0 +1,149 @@
+/* odyssey.h — C ABI of the B200-native Odyssey hot path (arXiv 1601.02063).
+ *
+ * One image-plane pixel = one photon traced backwards from the observer through Kerr spacetime in
+ * Boyer–Lindquist coordinates (§2.1, eqs. (1)-(15)), initial conditions
+ * of PAPER.md §2.2 (eqs. (18)-(26)), adaptive embedded 5th-order Runge–Kutta
+ * (PAPER.md:L90), with the radiative transfer of PAPER.md §2.3 (eqs. (2), (27)-(31),
+ * PAPER.md:L42-46, L149-171) advanced once per accepted step.  Every step of that path runs in the
+ * sm_100a kernels of paper_1601_02063_b200/csrc/; there is no CPU fallback.
+ *
+ * Conventions common to all calls
+ *   - Units: G = c = M = 1 for geometry; cgs for radiative quantities.
+ *   - Pixel grid: pixel (i, j), 0 <= i < nx, 0 <= j < ny, has image-plane coordinates
+ *       x = x_min + (i + 1/2)(x_max - x_min)/nx   (alpha, to the observer's right),
+ *       y = y_min + (j + 1/2)(y_max - y_min)/ny   (beta, along the projected spin axis);
+ *     per-pixel arrays are row-major [j][i] (index j*nx + i), structure-of-arrays, one array per
+ *     quantity.  Per-frequency images are [k][j][i].
+ *   - DEVICE entry points (no suffix): every output pointer is a caller-owned DEVICE buffer on the
+ *     current CUDA device; a NULL output pointer means "do not write this quantity".  The call
+ *     enqueues its work on `cuda_stream` (a cudaStream_t passed as void*, NULL = default stream)
+ *     and returns without synchronising; the caller synchronises before reading.
+ *   - HOST entry points (suffix _host): same arguments but every output pointer is HOST memory; the
+ *     call allocates device scratch, runs the same kernels, copies the results back and returns
+ *     after the copies have completed (synchronous).
+ *   - The structs and the frequency list are always HOST memory, read during the call only.
+ *   - Return value: ODYSSEY_OK (0) or a negative odyssey_status.  After a failure
+ *     odyssey_last_error() returns a static, thread-local, NUL-terminated description.
+ *     Nothing is printed, nothing throws.
+ *   - The library owns only a small ring of work-queue counters per device (allocated lazily,
+ *     released by odyssey_shutdown()).
+ */
+#ifndef ODYSSEY_H_
+#define ODYSSEY_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum odyssey_status {
+    ODYSSEY_OK = 0,
+    ODYSSEY_ERR_INVALID_ARGUMENT = -1, /* |a| >= 1, nx/ny <= 0, rtol <= 0, nf outside [1,32], unknown kind/tableau, NULL struct */
+    ODYSSEY_ERR_CUDA = -2,             /* a CUDA runtime call or the launch failed; text in odyssey_last_error() */
+    ODYSSEY_ERR_UNSUPPORTED_DEVICE = -3 /* current device is not compute capability 10.x */
+} odyssey_status;
+
+/* Ray outcome written to `flag` ("captured"; L223 disk; BASELINE.json:configs[2] optical depth). */
+enum {
+    ODYSSEY_FLAG_ESCAPED = 0,  /* p_r > 0 and r >= r_esc; final state located ON r = r_esc          */
+    ODYSSEY_FLAG_CAPTURED = 1, /* r <= r_h + horizon_eps; final state located ON that radius         */
+    ODYSSEY_FLAG_DISK = 2,     /* kind 1: first equatorial crossing with r_in <= r <= r_out           */
+    ODYSSEY_FLAG_OPAQUE = 3,   /* kind 2: every frequency has tau > tau_max                           */
+    ODYSSEY_FLAG_MAXSTEP = 4   /* max_attempts Runge–Kutta attempts used                              */
+};
+
+enum { ODYSSEY_TABLEAU_RKF45 = 0, ODYSSEY_TABLEAU_CASH_KARP = 1 };
+enum { ODYSSEY_KIND_NONE = 0, ODYSSEY_KIND_THIN_DISK = 1, ODYSSEY_KIND_RIAF = 2 };
+#define ODYSSEY_MAX_FREQ 32
+
+/* The observer, the image plane and the integrator controls. */
+typedef struct odyssey_scene {
+    double a;                  /* spin, |a| < 1                                                  */
+    double r_obs;              /* observer distance (PAPER.md:L106 uses 10^3)                    */
+    double theta_obs, phi_obs; /* observer inclination and azimuth, radians                      */
+    double x_min, x_max, y_min, y_max; /* image-plane extent (edges, not centres)               */
+    int32_t nx, ny;            /* resolution                                                     */
+    double rtol;               /* per-step tolerance of the scaled max-norm error                */
+    int32_t tableau, pad0;     /* ODYSSEY_TABLEAU_*                                              */
+    double h0;                 /* first trial step in affine parameter                           */
+    double horizon_eps;        /* capture radius = r_h + horizon_eps                             */
+    double r_esc;              /* escape radius                                                  */
+    int32_t max_attempts, pad1;
+} odyssey_scene;
+
+/* Emission model (PAPER.md:L223 thin disk; L268-292 thermal synchrotron; BASELINE.json:configs[1..2]). */
+typedef struct odyssey_model {
+    int32_t kind;              /* ODYSSEY_KIND_*                                                 */
+    int32_t nbins;             /* kind 1: number of g bins of the line profile (0 = none)        */
+    double r_in, r_out;        /* kind 1: disk radii; r_in <= 0 means r_isco(a)                  */
+    double emis_index;         /* kind 1: emissivity ∝ r^-emis_index                             */
+    double mbh_msun;           /* kind 2: black-hole mass in solar masses (sets r_g in cm)       */
+    double n0, n_index;        /* kind 2: n_e = n0 (r/r_h)^n_index exp(-cos^2θ / (2 h_over_r^2)) */
+    double T0, T_index;        /* kind 2: T_e = T0 (r/r_h)^T_index                               */
+    double h_over_r, beta;     /* kind 2: scale height, magnetisation B^2/8π = n_e m_p c^2/(6 β r) */
+    double r_rt_out;           /* kind 2: no emission outside this radius        */
+    double tau_max;            /* kind 2: a frequency is frozen once tau > tau_max               */
+    double j_scale;            /* kind 2: 1 = per-steradian emissivity; 4π reproduces eq. (37) as printed */
+    double g_lo, g_hi;         /* kind 1: histogram range in g                                   */
+    double g_power;            /* kind 1: pixel value = g^g_power r_e^-emis_index                */
+} odyssey_model;
+
+/* Geodesics only (BASELINE.json:configs[0]; §2.1-2.2).  Per pixel: outcome flag, the
+ * final Boyer–Lindquist position (r, theta, phi) — located on the stopping surface — and the
+ * number of attempted and accepted Runge–Kutta steps ("total number of steps").  */
+int odyssey_trace_geodesics(const odyssey_scene* scene,
+                            int32_t* flag, double* r, double* theta, double* phi,
+                            int32_t* n_attempt, int32_t* n_accept, void* cuda_stream);
+
+/* One observed frequency nu_hz (ignored by kind 0/1).
+ *   kind 1 (eq. (2)): image = g^g_power r_e^-emis_index, aux0 = g, aux1 = r_e of the
+ *     first disk crossing (0 where the ray misses); hist[nbins] += image × pixel area in the bin of g
+ *     (hist is overwritten, not accumulated across calls).
+ *   kind 2 (eqs. (30),(31),(37)-(39)): image = I_nu = nu^3 × invariant intensity (erg s^-1 cm^-2
+ *     Hz^-1 sr^-1), aux0 = optical depth tau, aux1 = 0.
+ *   kind 0: image = aux0 = aux1 = 0; flags and step counts as odyssey_trace_geodesics.           */
+int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model, double nu_hz,
+                         double* image, double* aux0, double* aux1, int32_t* flag,
+                         int32_t* n_attempt, double* hist, void* cuda_stream);
+
+/* nf <= 32 observed frequencies integrated simultaneously along each geodesic (kind 2 only;
+ * BASELINE.json:configs[3]).  images[nf][ny][nx] = I_nu; nuLnu[nf] = 4π nu r_g^2 Δx Δy Σ_pixels I_nu
+ * (erg/s; the distance cancels).  nu_hz_host is HOST memory.                                      */
+int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* model,
+                            const double* nu_hz_host, int nf,
+                            double* images, double* nuLnu, int32_t* flag, int32_t* n_attempt,
+                            void* cuda_stream);
+
+/* Host-buffer variants: identical semantics, every output pointer is HOST memory, synchronous. */
+int odyssey_trace_geodesics_host(const odyssey_scene* scene,
+                                 int32_t* flag, double* r, double* theta, double* phi,
+                                 int32_t* n_attempt, int32_t* n_accept);
+int odyssey_render_image_host(const odyssey_scene* scene, const odyssey_model* model, double nu_hz,
+                              double* image, double* aux0, double* aux1, int32_t* flag,
+                              int32_t* n_attempt, double* hist);
+int odyssey_render_spectrum_host(const odyssey_scene* scene, const odyssey_model* model,
+                                 const double* nu_hz_host, int nf,
+                                 double* images, double* nuLnu, int32_t* flag, int32_t* n_attempt);
+
+/* FP64 peak probe (BASELINE.json:north_star "measured by a DFMA microbenchmark in the same run"):
+ * enqueues a kernel in which every thread runs `iters` rounds of 16 independent DFMA chains
+ * on a full-occupancy grid.  *flop_host receives the number of floating-point operations the launch
+ * performs (2 per DFMA); sink is a DEVICE buffer of at least 8 bytes.  The caller times it.     */
+int odyssey_fp64_peak_probe(int iters, double* sink, double* flop_host, void* cuda_stream);
+
+/* Kernel facts for reports: registers per thread, local (spill) bytes per thread, static shared
+ * bytes, threads per block and resident blocks per SM of the kernel that serves (kind, nf > 1).  */
+int odyssey_kernel_info(int kind, int spectrum, int tableau, int32_t* regs, int32_t* local_bytes,
+                        int32_t* threads_per_block, int32_t* blocks_per_sm, int32_t* n_sm);
+
+/* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
+long long odyssey_launch_count(void);
+
+const char* odyssey_last_error(void);
+void odyssey_shutdown(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ODYSSEY_H_ */

@@ -1,0 +1,362 @@
+// odyssey_api.cu — the C ABI of include/odyssey.h: argument checks, the constant block, launches.
+// No torch types, no CPU fallback: every entry point either enqueues the sm_100a kernels of
+// odyssey_kernels.cuh or returns an error code.
+#include <cuda_runtime.h>
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+
+#include "../../include/odyssey.h"
+#include "odyssey_kernels.cuh"
+
+namespace {
+
+using namespace ody;
+
+// ---- physical constants, cgs (CODATA 2018; IAU nominal GM_sun) ---------------------------------
+constexpr double kC = 2.99792458e10, kGMsun = 1.3271244e26, kH = 6.62607015e-27, kKB = 1.380649e-16;
+constexpr double kMe = 9.1093837015e-28, kMp = 1.67262192369e-24, kE = 4.80320471257e-10;
+constexpr double kPi = 3.14159265358979323846;
+
+thread_local char g_err[512] = "";
+std::atomic<long long> g_launches{0};
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap; va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                             \
+    do { cudaError_t e_ = (expr);                                                                  \
+         if (e_ != cudaSuccess) return fail(ODYSSEY_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
+
+// ---- per-device library state: SM count and a ring of queue counters --------------------------
+constexpr int MAX_DEV = 16, RING = 64;
+struct DevState { bool ready = false; int n_sm = 0; unsigned long long* ring = nullptr; unsigned next = 0; };
+DevState g_dev[MAX_DEV];
+std::mutex g_mu;
+
+int device_state(DevState** out, int* dev_out) {
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEV) return fail(ODYSSEY_ERR_CUDA, "device index %d out of range", dev);
+    std::lock_guard<std::mutex> lk(g_mu);
+    DevState& D = g_dev[dev];
+    if (!D.ready) {
+        cudaDeviceProp prop;
+        CUDA_TRY(cudaGetDeviceProperties(&prop, dev));
+        if (prop.major != 10)
+            return fail(ODYSSEY_ERR_UNSUPPORTED_DEVICE, "device %d is sm_%d%d; this library is built for sm_100a only", dev, prop.major, prop.minor);
+        D.n_sm = prop.multiProcessorCount;
+        CUDA_TRY(cudaMalloc(&D.ring, RING * sizeof(unsigned long long)));
+        D.ready = true;
+    }
+    *out = &D; if (dev_out) *dev_out = dev;
+    return ODYSSEY_OK;
+}
+
+unsigned long long* next_counter(DevState* D) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    return D->ring + (D->next++ % RING);
+}
+
+// ---- Kerr constants (Bardeen, Press & Teukolsky 1972, cited PAPER.md:L223) -----------------------
+double isco_radius(double a) {
+    const double z1 = 1.0 + std::cbrt(1.0 - a * a) * (std::cbrt(1.0 + a) + std::cbrt(1.0 - a));
+    const double z2 = std::sqrt(3.0 * a * a + z1 * z1);
+    return 3.0 + z2 - (a >= 0.0 ? 1.0 : -1.0) * std::sqrt((3.0 - z1) * (3.0 + z1 + 2.0 * z2));
+}
+
+int check_scene(const odyssey_scene* S) {
+    if (!S) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "scene is NULL");
+    if (!(std::fabs(S->a) < 1.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spin |a| = %g must be < 1", S->a);
+    if (S->nx <= 0 || S->ny <= 0) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nx = %d, ny = %d must be positive", S->nx, S->ny);
+    if ((long long)S->nx * S->ny > (1LL << 30)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nx*ny exceeds 2^30 pixels");
+    if (!(S->rtol > 0.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "rtol = %g must be > 0", S->rtol);
+    if (S->tableau != ODYSSEY_TABLEAU_RKF45 && S->tableau != ODYSSEY_TABLEAU_CASH_KARP)
+        return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown tableau %d", S->tableau);
+    if (!(S->r_obs > 0.0) || !(S->h0 > 0.0) || !(S->r_esc > 0.0) || !(S->horizon_eps >= 0.0) || S->max_attempts <= 0)
+        return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "r_obs, h0, r_esc, max_attempts must be positive and horizon_eps >= 0");
+    if (!(S->x_max > S->x_min) || !(S->y_max > S->y_min))
+        return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "image-plane extent is empty");
+    return ODYSSEY_OK;
+}
+
+int check_model(const odyssey_model* M) {
+    if (!M) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "model is NULL");
+    if (M->kind < ODYSSEY_KIND_NONE || M->kind > ODYSSEY_KIND_RIAF) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown model kind %d", M->kind);
+    if (M->kind == ODYSSEY_KIND_THIN_DISK) {
+        if (M->nbins < 0 || M->nbins > 4096) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nbins = %d outside [0, 4096]", M->nbins);
+        if (M->nbins > 0 && !(M->g_hi > M->g_lo)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "g_hi must exceed g_lo");
+    }
+    if (M->kind == ODYSSEY_KIND_RIAF) {
+        if (!(M->mbh_msun > 0.0) || !(M->h_over_r > 0.0) || !(M->beta > 0.0) || !(M->T0 > 0.0) || !(M->n0 >= 0.0))
+            return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "RIAF parameters mbh_msun, h_over_r, beta, T0 must be positive");
+    }
+    return ODYSSEY_OK;
+}
+
+void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* nu, int nf, Params* P) {
+    std::memset(P, 0, sizeof(*P));
+    P->a = S.a; P->a2 = S.a * S.a;
+    P->r_obs = S.r_obs; P->R_obs = std::sqrt(S.r_obs * S.r_obs + S.a * S.a);
+    P->sin_obs = std::sin(S.theta_obs); P->cos_obs = std::cos(S.theta_obs);
+    P->sin_pobs = std::sin(S.phi_obs); P->cos_pobs = std::cos(S.phi_obs); P->phi_obs = S.phi_obs;
+    P->x_min = S.x_min; P->x_span = S.x_max - S.x_min; P->y_min = S.y_min; P->y_span = S.y_max - S.y_min;
+    P->pix_area = (P->x_span / S.nx) * (P->y_span / S.ny);
+    P->rtol = S.rtol; P->h0 = S.h0;
+    P->r_h = 1.0 + std::sqrt(1.0 - S.a * S.a);
+    P->r_cap = P->r_h + S.horizon_eps; P->r_esc = S.r_esc;
+    P->nx = S.nx; P->ny = S.ny; P->max_attempts = S.max_attempts;
+    P->tiles_x = (S.nx + TILE_W - 1) / TILE_W;
+    const long long tiles_y = (S.ny + TILE_H - 1) / TILE_H;
+    P->n_queue = (long long)P->tiles_x * tiles_y * (TILE_W * TILE_H);
+    // circular equatorial orbit at the ISCO: specific energy and angular momentum
+    P->r_isco = isco_radius(S.a);
+    {
+        const double r = P->r_isco, sr = std::sqrt(r);
+        const double den = std::pow(r, 0.75) * std::sqrt(r * sr - 3.0 * sr + 2.0 * S.a);
+        P->E_isco = (r * sr - 2.0 * sr + S.a) / den;
+        P->L_isco = (r * r - 2.0 * S.a * sr + S.a * S.a) / den;
+    }
+    P->kind = M ? M->kind : 0;
+    P->nf = nf;
+    if (!M) return;
+    if (M->kind == ODYSSEY_KIND_THIN_DISK) {
+        P->r_in = (M->r_in > 0.0) ? M->r_in : P->r_isco;
+        P->r_out = M->r_out; P->emis_index = M->emis_index; P->g_power = M->g_power;
+        P->g_lo = M->g_lo; P->g_hi = M->g_hi; P->nbins = M->nbins;
+    }
+    if (M->kind == ODYSSEY_KIND_RIAF) {
+        P->n0 = M->n0; P->n_index = M->n_index; P->T0 = M->T0; P->T_index = M->T_index;
+        P->inv_2h2 = 1.0 / (2.0 * M->h_over_r * M->h_over_r);
+        P->B2_coef = 8.0 * kPi * kMp * kC * kC / (6.0 * M->beta);
+        P->theta_per_K = kKB / (kMe * kC * kC);
+        P->nuc_coef = 3.0 * kE / (4.0 * kPi * kMe * kC);
+        P->j_coef = M->j_scale * kE * kE / (std::sqrt(3.0) * kC);
+        P->planck_coef = 2.0 * kH / (kC * kC);
+        P->h_over_k = kH / kKB;
+        P->r_rt_out = M->r_rt_out; P->tau_max = M->tau_max;
+        P->rg_cm = kGMsun * M->mbh_msun / (kC * kC);
+        P->sed_coef = 4.0 * kPi * P->rg_cm * P->rg_cm * P->pix_area;
+        for (int k = 0; k < nf && k < MAX_FREQ; ++k) { P->nu[k] = nu[k]; P->nu3[k] = nu[k] * nu[k] * nu[k]; }
+    }
+}
+
+// ---- kernel table ------------------------------------------------------------------------------
+constexpr int NT_MAIN = 128, MINB_MAIN = 3;     // 168 registers per thread at most
+constexpr int NT_SPEC = 160, MINB_SPEC = 1;     // 5 x 32 x 160 x 8 B = 200 KiB of accumulators
+
+typedef void (*KernelFn)(const Params, const Outputs);
+
+KernelFn pick_kernel(int kind, bool spec, int tab) {
+    if (spec) return tab ? odyssey_kernel<2, 1, true, NT_SPEC, MINB_SPEC> : odyssey_kernel<2, 0, true, NT_SPEC, MINB_SPEC>;
+    switch (kind) {
+        case 0: return tab ? odyssey_kernel<0, 1, false, NT_MAIN, MINB_MAIN> : odyssey_kernel<0, 0, false, NT_MAIN, MINB_MAIN>;
+        case 1: return tab ? odyssey_kernel<1, 1, false, NT_MAIN, MINB_MAIN> : odyssey_kernel<1, 0, false, NT_MAIN, MINB_MAIN>;
+        default: return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_MAIN> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_MAIN>;
+    }
+}
+
+size_t smem_bytes(int kind, bool spec, int nf, int nbins) {
+    if (spec) return (size_t)(5 * nf * NT_SPEC + MAX_FREQ) * sizeof(double);
+    if (kind == 1) return (size_t)(nbins > 0 ? nbins : 1) * sizeof(double);
+    return 0;
+}
+
+int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
+    DevState* D = nullptr;
+    int rc = device_state(&D, nullptr);
+    if (rc) return rc;
+    KernelFn fn = pick_kernel(P.kind, spec, tab);
+    const int nt = spec ? NT_SPEC : NT_MAIN;
+    const size_t sm = smem_bytes(P.kind, spec, P.nf, P.nbins);
+    if (sm > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    int per_sm = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, nt, sm));
+    if (per_sm < 1) return fail(ODYSSEY_ERR_CUDA, "kernel does not fit on an SM (shared memory %zu B)", sm);
+    // persistent grid: every SM full, but no more blocks than there are queue tiles to hand out
+    long long blocks = (long long)D->n_sm * per_sm;
+    const long long warps_needed = P.n_queue / 32;
+    const long long blocks_needed = (warps_needed + nt / 32 - 1) / (nt / 32);
+    if (blocks > blocks_needed) blocks = blocks_needed;
+    if (blocks < 1) blocks = 1;
+    O.queue = next_counter(D);
+    CUDA_TRY(cudaMemsetAsync(O.queue, 0, sizeof(unsigned long long), st));
+    if (O.hist && P.nbins > 0) CUDA_TRY(cudaMemsetAsync(O.hist, 0, sizeof(double) * P.nbins, st));
+    if (O.nuLnu) CUDA_TRY(cudaMemsetAsync(O.nuLnu, 0, sizeof(double) * P.nf, st));
+    void* args[] = {(void*)&P, (void*)&O};
+    CUDA_TRY(cudaLaunchKernel((const void*)fn, dim3((unsigned)blocks), dim3(nt), args, sm, st));
+    g_launches.fetch_add(1);
+    return ODYSSEY_OK;
+}
+
+Outputs no_outputs() { Outputs O; std::memset(&O, 0, sizeof(O)); return O; }
+
+}  // namespace
+
+// ---- host-buffer variants: device scratch, same kernels, copies back, synchronous -------------
+namespace {
+struct Scratch {
+    void* dev[12]; void* host[12]; size_t bytes[12]; int n = 0;
+    ~Scratch() { for (int i = 0; i < n; ++i) if (dev[i]) cudaFree(dev[i]); }
+    template <class T> int add(T* host_ptr, size_t count, T** out) {
+        *out = nullptr;
+        if (!host_ptr) return ODYSSEY_OK;
+        void* d = nullptr;
+        CUDA_TRY(cudaMalloc(&d, count * sizeof(T)));
+        dev[n] = d; host[n] = host_ptr; bytes[n] = count * sizeof(T); ++n;
+        *out = (T*)d;
+        return ODYSSEY_OK;
+    }
+    int copy_back() {
+        for (int i = 0; i < n; ++i) CUDA_TRY(cudaMemcpyAsync(host[i], dev[i], bytes[i], cudaMemcpyDeviceToHost, 0));
+        CUDA_TRY(cudaStreamSynchronize(0));
+        return ODYSSEY_OK;
+    }
+};
+#define TRY(expr) do { int rc_ = (expr); if (rc_) return rc_; } while (0)
+}  // namespace
+
+// ================================================================================================
+// extern "C" entry points (include/odyssey.h)
+// ================================================================================================
+extern "C" {
+
+int odyssey_trace_geodesics(const odyssey_scene* scene, int32_t* flag, double* r, double* theta, double* phi,
+                            int32_t* n_attempt, int32_t* n_accept, void* cuda_stream) {
+    int rc = check_scene(scene);
+    if (rc) return rc;
+    Params P; fill_params(*scene, nullptr, nullptr, 0, &P);
+    Outputs O = no_outputs();
+    O.flag = flag; O.r = r; O.th = theta; O.ph = phi; O.n_attempt = n_attempt; O.n_accept = n_accept;
+    return launch(P, O, false, scene->tableau, (cudaStream_t)cuda_stream);
+}
+
+int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model, double nu_hz,
+                         double* image, double* aux0, double* aux1, int32_t* flag, int32_t* n_attempt,
+                         double* hist, void* cuda_stream) {
+    int rc = check_scene(scene);
+    if (rc) return rc;
+    rc = check_model(model);
+    if (rc) return rc;
+    if (model->kind == ODYSSEY_KIND_RIAF && !(nu_hz > 0.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz = %g must be > 0", nu_hz);
+    Params P; fill_params(*scene, model, &nu_hz, 1, &P);
+    Outputs O = no_outputs();
+    O.image = image; O.aux0 = aux0; O.aux1 = aux1; O.flag = flag; O.n_attempt = n_attempt;
+    O.hist = (model->kind == ODYSSEY_KIND_THIN_DISK && model->nbins > 0) ? hist : nullptr;
+    return launch(P, O, false, scene->tableau, (cudaStream_t)cuda_stream);
+}
+
+int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* model, const double* nu_hz_host, int nf,
+                            double* images, double* nuLnu, int32_t* flag, int32_t* n_attempt, void* cuda_stream) {
+    int rc = check_scene(scene);
+    if (rc) return rc;
+    rc = check_model(model);
+    if (rc) return rc;
+    if (model->kind != ODYSSEY_KIND_RIAF) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode needs model kind 2 (RIAF), got %d", model->kind);
+    if (nf < 1 || nf > ODYSSEY_MAX_FREQ) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nf = %d outside [1, %d]", nf, ODYSSEY_MAX_FREQ);
+    if (!nu_hz_host) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz_host is NULL");
+    for (int k = 0; k < nf; ++k)
+        if (!(nu_hz_host[k] > 0.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz_host[%d] = %g must be > 0", k, nu_hz_host[k]);
+    Params P; fill_params(*scene, model, nu_hz_host, nf, &P);
+    Outputs O = no_outputs();
+    O.images = images; O.nuLnu = nuLnu; O.flag = flag; O.n_attempt = n_attempt;
+    return launch(P, O, true, scene->tableau, (cudaStream_t)cuda_stream);
+}
+
+// ---- host-buffer variants (Scratch defined above) ---------------------------------------------
+
+int odyssey_trace_geodesics_host(const odyssey_scene* scene, int32_t* flag, double* r, double* theta, double* phi,
+                                 int32_t* n_attempt, int32_t* n_accept) {
+    TRY(check_scene(scene));
+    const size_t n = (size_t)scene->nx * scene->ny;
+    Scratch S; int32_t *dflag, *datt, *dacc; double *dr, *dth, *dph;
+    TRY(S.add(flag, n, &dflag)); TRY(S.add(r, n, &dr)); TRY(S.add(theta, n, &dth)); TRY(S.add(phi, n, &dph));
+    TRY(S.add(n_attempt, n, &datt)); TRY(S.add(n_accept, n, &dacc));
+    TRY(odyssey_trace_geodesics(scene, dflag, dr, dth, dph, datt, dacc, nullptr));
+    return S.copy_back();
+}
+
+int odyssey_render_image_host(const odyssey_scene* scene, const odyssey_model* model, double nu_hz,
+                              double* image, double* aux0, double* aux1, int32_t* flag, int32_t* n_attempt, double* hist) {
+    TRY(check_scene(scene)); TRY(check_model(model));
+    const size_t n = (size_t)scene->nx * scene->ny;
+    Scratch S; double *dimg, *da0, *da1, *dhist; int32_t *dflag, *datt;
+    TRY(S.add(image, n, &dimg)); TRY(S.add(aux0, n, &da0)); TRY(S.add(aux1, n, &da1));
+    TRY(S.add(flag, n, &dflag)); TRY(S.add(n_attempt, n, &datt));
+    TRY(S.add((model->kind == ODYSSEY_KIND_THIN_DISK && model->nbins > 0) ? hist : nullptr, (size_t)model->nbins, &dhist));
+    TRY(odyssey_render_image(scene, model, nu_hz, dimg, da0, da1, dflag, datt, dhist, nullptr));
+    return S.copy_back();
+}
+
+int odyssey_render_spectrum_host(const odyssey_scene* scene, const odyssey_model* model, const double* nu_hz_host, int nf,
+                                 double* images, double* nuLnu, int32_t* flag, int32_t* n_attempt) {
+    TRY(check_scene(scene)); TRY(check_model(model));
+    if (nf < 1 || nf > ODYSSEY_MAX_FREQ) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nf = %d outside [1, %d]", nf, ODYSSEY_MAX_FREQ);
+    const size_t n = (size_t)scene->nx * scene->ny;
+    Scratch S; double *dimg, *dsed; int32_t *dflag, *datt;
+    TRY(S.add(images, n * nf, &dimg)); TRY(S.add(nuLnu, (size_t)nf, &dsed));
+    TRY(S.add(flag, n, &dflag)); TRY(S.add(n_attempt, n, &datt));
+    TRY(odyssey_render_spectrum(scene, model, nu_hz_host, nf, dimg, dsed, dflag, datt, nullptr));
+    return S.copy_back();
+}
+
+// ---- probes and bookkeeping ---------------------------------------------------------------------
+int odyssey_fp64_peak_probe(int iters, double* sink, double* flop_host, void* cuda_stream) {
+    if (iters <= 0 || !sink) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "iters must be > 0 and sink non-NULL");
+    DevState* D = nullptr;
+    TRY(device_state(&D, nullptr));
+    const int blocks = D->n_sm * 8, threads = 256;                    // 2048 resident threads per SM
+    dfma_probe_kernel<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>(iters, sink);
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+    if (flop_host) *flop_host = 2.0 * PROBE_DFMA_PER_ITER * (double)iters * (double)blocks * threads;
+    return ODYSSEY_OK;
+}
+
+int odyssey_kernel_info(int kind, int spectrum, int tableau, int32_t* regs, int32_t* local_bytes,
+                        int32_t* threads_per_block, int32_t* blocks_per_sm, int32_t* n_sm) {
+    if (kind < 0 || kind > 2 || (tableau != 0 && tableau != 1)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown kind/tableau");
+    DevState* D = nullptr;
+    TRY(device_state(&D, nullptr));
+    const bool spec = spectrum != 0;
+    KernelFn fn = pick_kernel(spec ? 2 : kind, spec, tableau);
+    cudaFuncAttributes at;
+    CUDA_TRY(cudaFuncGetAttributes(&at, (const void*)fn));
+    const int nt = spec ? NT_SPEC : NT_MAIN;
+    const size_t sm = smem_bytes(spec ? 2 : kind, spec, ODYSSEY_MAX_FREQ, 200);
+    if (sm > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    int per_sm = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, nt, sm));
+    if (regs) *regs = at.numRegs;
+    if (local_bytes) *local_bytes = (int32_t)at.localSizeBytes;
+    if (threads_per_block) *threads_per_block = nt;
+    if (blocks_per_sm) *blocks_per_sm = per_sm;
+    if (n_sm) *n_sm = D->n_sm;
+    return ODYSSEY_OK;
+}
+
+long long odyssey_launch_count(void) { return g_launches.load(); }
+
+const char* odyssey_last_error(void) { return g_err; }
+
+void odyssey_shutdown(void) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    int cur = 0;
+    if (cudaGetDevice(&cur) != cudaSuccess) return;
+    for (int d = 0; d < MAX_DEV; ++d) {
+        if (!g_dev[d].ready) continue;
+        cudaSetDevice(d);
+        cudaFree(g_dev[d].ring);
+        g_dev[d] = DevState();
+    }
+    cudaSetDevice(cur);
+}
+
+}  // extern "C"

@@ -1,0 +1,265 @@
+// odyssey_kernels.cuh — the fused geodesic + radiative-transfer kernel of the Odyssey hot path for
+// sm_100a (B200).  One lane = one photon = one image-plane pixel, but unlike
+// the paper's static "Grid by Grid" launch (eq. (32), written for a Kepler card)
+// the kernel is PERSISTENT: every lane pulls its next pixel from an atomic work queue as soon as
+// its ray ends (horizon capture, escape, disk hit, optical-depth cutoff), so warps stay full.
+//
+// Lane life cycle (one trip round the main loop = one Runge–Kutta attempt for every live lane):
+//   refill  : lanes without a ray ballot; the leader takes popc(ballot) queue slots with ONE
+//             atomicAdd; slot q -> tile q/32 (8x4 pixels, row-major tiles) -> pixel; init_ray.
+//   attempt : stages 2..6 from (y, k1, h); the first slope k1 = f(y) is cached, so a rejected
+//             attempt or a re-attempt of the event location costs 5 right-hand sides, not 6.
+//   control : scaled max-norm error vs rtol; reject -> shrink h; accept -> h_next.
+//   events  : equatorial crossing (thin disk), capture, escape.  The event LOCATION (Newton on h,
+//             re-taking the step from y) is a lane MODE, not an inner loop: a locating lane simply
+//             makes its next attempt with the corrected h alongside its warp-mates' normal attempts.
+//   commit  : radiative-transfer update over the step actually taken (eqs. (30), (31)), state
+//             advance, outputs + release of the lane when the ray has ended.
+//
+// All per-ray state lives in registers; the spectrum variant keeps its 5 x nf per-frequency
+// accumulators in shared memory laid out [quantity][frequency][thread] (bank-conflict free).
+#pragma once
+#include <cuda_runtime.h>
+#include "params.h"
+#include "geodesic.cuh"
+#include "emission.cuh"
+
+namespace ody {
+
+constexpr int M_NORMAL = 0, M_EQ = 1, M_CAP = 2, M_ESC = 3;       // lane modes
+constexpr int F_ESCAPED = 0, F_CAPTURED = 1, F_DISK = 2, F_OPAQUE = 3, F_MAXSTEP = 4;
+constexpr unsigned FULL = 0xffffffffu;
+constexpr double HALF_PI = 1.57079632679489661923;
+
+// capture / escape test on a candidate end state (reading J)
+__device__ __forceinline__ int radial_event(const Params& P, const State& yn) {
+    if (yn.r <= P.r_cap) return M_CAP;
+    if (yn.pr > 0.0 && yn.r >= P.r_esc) return M_ESC;
+    return M_NORMAL;
+}
+
+template <int KIND, int TAB, bool SPEC, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB)
+odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs O) {
+    extern __shared__ double smem[];
+    const int lane = threadIdx.x & 31;
+    const int nf = SPEC ? P.nf : 1;
+    // shared layout: SPEC: [5][nf][NT] accumulators then sed[MAX_FREQ]; KIND 1: hist[nbins]
+    double* const sm_acc = smem;
+    double* const sm_red = SPEC ? smem + 5 * nf * NT : smem;
+    if (SPEC) { for (int k = threadIdx.x; k < MAX_FREQ; k += NT) sm_red[k] = 0.0; }
+    if (KIND == 1) { for (int k = threadIdx.x; k < P.nbins; k += NT) sm_red[k] = 0.0; }
+    if (SPEC || KIND == 1) __syncthreads();
+#define ACC(q, k) sm_acc[((q) * nf + (k)) * NT + threadIdx.x]      // q: 0 tau, 1 T, 2 I, 3 a0, 4 e0
+
+    const double a = P.a, a2 = P.a2;
+    bool active = false, exhausted = false, on_eq = false;
+    int pix = 0, n_att = 0, n_acc = 0, mode = M_NORMAL, loc_it = 0;
+    State y; Slope k1;
+    double L = 0.0, h_try = 0.0, h_next = 0.0, cos_y = 0.0;
+    double tau = 0.0, Tr = 1.0, Inu = 0.0, a0 = 0.0, e0 = 0.0;      // single-frequency RT state
+    double g_disk = 0.0, r_e = 0.0;
+    y.r = y.th = y.ph = y.pr = y.pth = 0.0;
+    k1.r = k1.th = k1.ph = k1.pr = k1.pth = 0.0;
+
+    for (;;) {
+        // ------------------------------------------------------------------ refill from the queue
+        const unsigned need = __ballot_sync(FULL, !active && !exhausted);
+        if (need) {
+            const int leader = __ffs(need) - 1;
+            unsigned long long base = 0;
+            if (lane == leader) base = atomicAdd(O.queue, (unsigned long long)__popc(need));
+            base = __shfl_sync(FULL, base, leader);
+            if (!active && !exhausted) {
+                const long long q = (long long)base + __popc(need & ((1u << lane) - 1u));
+                if (q >= P.n_queue) {
+                    exhausted = true;
+                } else {
+                    const int tile = (int)(q >> 5), w = (int)(q & 31);
+                    const int i = (tile % P.tiles_x) * TILE_W + (w & (TILE_W - 1));
+                    const int j = (tile / P.tiles_x) * TILE_H + (w / TILE_W);
+                    if (i < P.nx && j < P.ny) {
+                        const double x = P.x_min + (i + 0.5) * P.x_span / P.nx;      // pixel centres (reading K)
+                        const double yy = P.y_min + (j + 0.5) * P.y_span / P.ny;
+                        init_ray(P, x, yy, y, L);
+                        double s0, c0;
+                        geodesic_rhs(a, a2, L, y.r, y.th, y.pr, y.pth, k1, s0, c0);
+                        cos_y = c0;
+                        pix = j * P.nx + i;
+                        n_att = 0; n_acc = 0; mode = M_NORMAL; loc_it = 0; on_eq = false;
+                        h_try = P.h0; g_disk = 0.0; r_e = 0.0;
+                        if (KIND == 2) {
+                            RtPoint pt; rt_point(P, L, y.r, s0, c0, y.pr, pt);
+                            if (SPEC) {
+                                for (int k = 0; k < nf; ++k) {
+                                    double ac, ec; rt_coefficients(P, pt, P.nu[k], ac, ec);
+                                    ACC(0, k) = 0.0; ACC(1, k) = 1.0; ACC(2, k) = 0.0; ACC(3, k) = ac; ACC(4, k) = ec;
+                                }
+                            } else {
+                                rt_coefficients(P, pt, P.nu[0], a0, e0);
+                                tau = 0.0; Tr = 1.0; Inu = 0.0;
+                            }
+                        }
+                        active = true;
+                    }
+                }
+            }
+        }
+        if (!__any_sync(FULL, active)) {
+            if (__all_sync(FULL, exhausted)) break;
+            continue;
+        }
+        if (!active) continue;
+
+        // ------------------------------------------------------------------ one attempt
+        int flag = -1;
+        if (mode == M_NORMAL && n_att >= P.max_attempts) {
+            flag = F_MAXSTEP;
+        } else {
+            State yn, ye;
+            rk_attempt<TAB>(a, a2, L, y, k1, h_try, yn, ye);
+            ++n_att;
+            if (mode == M_NORMAL) {
+                const double err = error_norm(y, ye, P.rtol);
+                if (!(err <= 1.0)) {                                   // reject (also NaN)
+                    h_try *= isfinite(err) ? fmax(0.1, 0.9 * rsqrt(sqrt(err))) : 0.1;
+                    continue;
+                }
+                ++n_acc;
+                h_next = h_try * ((err < 1.889568e-4) ? 5.0 : fmin(5.0, 0.9 * inv_fifth_root(err)));
+            } else {
+                ++loc_it;
+            }
+            // slopes at the candidate end state: next step's k1, the Newton derivative, sinθ/cosθ for the RT
+            Slope kn; double sn, cn;
+            geodesic_rhs(a, a2, L, yn.r, yn.th, yn.pr, yn.pth, kn, sn, cn);
+
+            if (mode == M_NORMAL) {                                    // fresh accepted step: detect events
+                int m = M_NORMAL;
+                if (KIND == 1) {
+                    if (!on_eq && cos_y * cn < 0.0) m = M_EQ;          // equatorial crossing (reading P)
+                    else on_eq = false;
+                }
+                if (m == M_NORMAL) m = radial_event(P, yn);
+                mode = m; loc_it = 0;
+            }
+            bool retake = false;
+            while (mode != M_NORMAL) {                                 // at most two passes (EQ then radial)
+                const double target = (mode == M_EQ) ? HALF_PI : ((mode == M_CAP) ? P.r_cap : P.r_esc);
+                const double f = ((mode == M_EQ) ? yn.th : yn.r) - target;
+                const double ftol = 1e-12 * fmax(1.0, fabs(target));
+                if (loc_it < LOCATE_MAX && fabs(f) > ftol) {           // Newton on the step size, re-take from y
+                    h_try -= f / ((mode == M_EQ) ? kn.th : kn.r);
+                    retake = true;
+                    break;
+                }
+                if (mode == M_EQ) {
+                    on_eq = true; mode = M_NORMAL;
+                    if (yn.r >= P.r_in && yn.r <= P.r_out && yn.r > P.r_cap) {
+                        flag = F_DISK; r_e = yn.r;
+                        double gam;
+                        if (flow_gamma(P, L, r_e, 1.0, 0.0, yn.pr, gam)) g_disk = gam;
+                    } else {
+                        mode = radial_event(P, yn); loc_it = 0;
+                    }
+                } else {
+                    flag = (mode == M_CAP) ? F_CAPTURED : F_ESCAPED;
+                    mode = M_NORMAL;
+                }
+            }
+            if (retake) continue;
+
+            // -------------------------------------------------------------- commit the step
+            if (KIND == 2) {
+                RtPoint pt; rt_point(P, L, yn.r, sn, cn, yn.pr, pt);
+                bool all_opaque = true;
+                if (SPEC) {
+                    for (int k = 0; k < nf; ++k) {
+                        double a1, e1; rt_coefficients(P, pt, P.nu[k], a1, e1);
+                        double tk = ACC(0, k), Tk = ACC(1, k), Ik = ACC(2, k);
+                        rt_update(ACC(3, k), a1, ACC(4, k), e1, h_try, P.tau_max, tk, Tk, Ik);
+                        ACC(0, k) = tk; ACC(1, k) = Tk; ACC(2, k) = Ik; ACC(3, k) = a1; ACC(4, k) = e1;
+                        if (!(tk > P.tau_max)) all_opaque = false;
+                    }
+                } else {
+                    double a1, e1; rt_coefficients(P, pt, P.nu[0], a1, e1);
+                    rt_update(a0, a1, e0, e1, h_try, P.tau_max, tau, Tr, Inu);
+                    a0 = a1; e0 = e1;
+                    all_opaque = (tau > P.tau_max);
+                }
+                if (flag < 0 && all_opaque) flag = F_OPAQUE;
+            }
+            y = yn; k1 = kn; cos_y = cn; h_try = h_next;
+        }
+
+        // ------------------------------------------------------------------ ray ended: outputs, release the lane
+        if (flag >= 0) {
+            if (O.flag) O.flag[pix] = flag;
+            if (O.r) O.r[pix] = y.r;
+            if (O.th) O.th[pix] = y.th;
+            if (O.ph) O.ph[pix] = y.ph;
+            if (O.n_attempt) O.n_attempt[pix] = n_att;
+            if (O.n_accept) O.n_accept[pix] = n_acc;
+            if (KIND == 0) {
+                if (O.image) O.image[pix] = 0.0;
+                if (O.aux0) O.aux0[pix] = 0.0;
+                if (O.aux1) O.aux1[pix] = 0.0;
+            } else if (KIND == 1) {
+                double val = 0.0;
+                if (flag == F_DISK && g_disk > 0.0) val = pow(g_disk, P.g_power) * pow(r_e, -P.emis_index);
+                if (O.image) O.image[pix] = val;
+                if (O.aux0) O.aux0[pix] = g_disk;
+                if (O.aux1) O.aux1[pix] = r_e;
+                if (O.hist && flag == F_DISK && g_disk >= P.g_lo && g_disk < P.g_hi) {    // line profile (reading Q)
+                    int b = (int)floor((g_disk - P.g_lo) / (P.g_hi - P.g_lo) * P.nbins);
+                    if (b >= P.nbins) b = P.nbins - 1;
+                    atomicAdd(&sm_red[b], val * P.pix_area);
+                }
+            } else if (!SPEC) {
+                if (O.image) O.image[pix] = P.nu3[0] * Inu;
+                if (O.aux0) O.aux0[pix] = tau;
+                if (O.aux1) O.aux1[pix] = 0.0;
+            } else {
+                const size_t npix = (size_t)P.nx * P.ny;
+                for (int k = 0; k < nf; ++k) {
+                    const double v = P.nu3[k] * ACC(2, k);
+                    if (O.images) O.images[(size_t)k * npix + pix] = v;
+                    if (O.nuLnu) atomicAdd(&sm_red[k], v);
+                }
+            }
+            active = false;
+        }
+    }
+#undef ACC
+    // ---------------------------------------------------------------------- block-level reductions
+    if (SPEC && O.nuLnu) {
+        __syncthreads();
+        for (int k = threadIdx.x; k < nf; k += NT) atomicAdd(&O.nuLnu[k], P.sed_coef * P.nu[k] * sm_red[k]);
+    }
+    if (KIND == 1 && O.hist) {
+        __syncthreads();
+        for (int k = threadIdx.x; k < P.nbins; k += NT) if (sm_red[k] != 0.0) atomicAdd(&O.hist[k], sm_red[k]);
+    }
+}
+
+// FP64 peak probe: 16 independent DFMA chains per thread (BASELINE.json:north_star).
+__global__ void __launch_bounds__(256) dfma_probe_kernel(int iters, double* sink) {
+    double v[16];
+    const double m = 1.0 - 1e-9 * (threadIdx.x & 7), c = 1e-9 * (blockIdx.x & 3);
+#pragma unroll
+    for (int q = 0; q < 16; ++q) v[q] = 1.0 + 0.001 * q + 1e-6 * threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int rep = 0; rep < 8; ++rep) {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) v[q] = fma(v[q], m, c);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) s += v[q];
+    if (s == 123.456) sink[0] = s;        // never true; keeps the chains alive
+}
+constexpr int PROBE_DFMA_PER_ITER = 16 * 8;
+
+}  // namespace ody
