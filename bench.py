@@ -1,0 +1,320 @@
+#!/usr/bin/env python
+"""bench.py — headline measurement of the Odyssey hot path on B200 (contract: see DESIGN.md §7).
+
+A *step* is one pass of the whole hot path — pixel → initial conditions → adaptive RK geodesic
+integration fused with the per-step radiative-transfer update → SoA stores — over one image of the
+throughput configuration C4 (BASELINE.json:configs[4]: a = 0.998, i = 85 deg, 4096 x 4096 = 16.8 M
+photons, RIAF at 230 GHz, FP64), through the C ABI (odyssey_render_image).
+
+Printed JSON line (rank 0):
+  metric/value    ns per photon per RK step = device time / total attempted RK steps (lower is better)
+  images_per_s    1 / step time (aggregate over ranks)
+  roofline        bound "alu": algorithmic FP64 flop / kernel time vs the DFMA peak
+                  measured in this same run by odyssey_fp64_peak_probe
+  e2e             the same metric through odyssey_render_image_host (host buffers, copies in the
+                  timed region)
+  cpu_baseline    the CPU oracle, as it stands, on a bounded strided sample of the same image plane
+
+`--impl reference` times the oracle alone (there is no reference implementation to install: the
+reference is a paper).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402
+
+METRIC = "ns per photon per RK step (FP64)"
+UNIT = "ns/photon/step"
+
+# Algorithmic FP64 work: flop per attempted RK step of the
+# geodesic system, and per radiative-transfer update (one per accepted step, single frequency).
+FLOP_PER_ATTEMPT_GEODESIC = 1500.0
+FLOP_PER_RT_UPDATE = 600.0
+
+
+def parse_args():
+    p = argparse.ArgumentParser()
+    p.add_argument("--gpus", type=int, default=1)
+    p.add_argument("--steps", type=int, default=5)
+    p.add_argument("--warmup", type=int, default=3)
+    p.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    p.add_argument("--n", type=int, default=4096, help="image side (C4 sweep: 1024, 2048, 4096)")
+    p.add_argument("--a", type=float, default=0.998, help="spin (C4 sweep: 0, 0.5, 0.9, 0.998)")
+    p.add_argument("--cpu-sample", type=int, default=320, help="side of the strided sub-grid the oracle is timed on")
+    p.add_argument("--no-cpu-baseline", action="store_true")
+    p.add_argument("--no-e2e", action="store_true")
+    return p.parse_args()
+
+
+def workload_name(n, a):
+    return f"C4: Kerr a={a:g}, i=85deg, {n}x{n} over +/-15M, r_obs=1000M, RIAF 230 GHz, RKF45 rtol 1e-8"
+
+
+# ---------------------------------------------------------------------------------------------------
+# clocks: sample nvidia-smi DURING the timed region (B200_PROFILING.md recipe)
+# ---------------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for row in self.rows:
+            f = [x.strip() for x in row.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------
+# the oracle legs (cpu_baseline and --impl reference): the only places bench.py executes oracle/
+# ---------------------------------------------------------------------------------------------------
+def time_oracle_sample(w, n_sub):
+    """One pass of the oracle over an n_sub x n_sub grid of pixel centres spanning the same image
+    plane as workload w.  Returns (seconds, attempted steps, rays, threads)."""
+    from oracle import binding as orc
+    sc = W.coarse_scene(w["scene"], n_sub)
+    t0 = time.perf_counter()
+    out = orc.render_image(sc, w["model"], w["nu"][0])
+    dt = time.perf_counter() - t0
+    return dt, int(out["n_attempt"].astype("int64").sum()), n_sub * n_sub, orc.num_threads()
+
+
+def cpu_baseline(w, n_sub):
+    dt, attempts, rays, threads = time_oracle_sample(w, n_sub)
+    return {"value": dt / attempts * 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{n_sub}x{n_sub} strided sub-grid of the same image plane, {rays} rays, "
+                      f"{attempts} attempted RK steps, {dt:.2f} s wall on {threads} threads",
+            "per_core_ns": dt * threads / attempts * 1e9}
+
+
+def run_reference(args):
+    """The reference arm: there is no reference code (the reference is a paper), so the oracle is timed."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import build as oracle_build
+    oracle_build.build()
+    w = W.C4(n=args.n, a=args.a)
+    n_sub = args.cpu_sample
+    for _ in range(min(args.warmup, 1)):
+        time_oracle_sample(w, 64)
+    tot_t, tot_att, threads, rays = 0.0, 0, 1, 0
+    for _ in range(args.steps):
+        dt, attempts, rays, threads = time_oracle_sample(w, n_sub)
+        tot_t += dt; tot_att += attempts
+    value = tot_t / tot_att * 1e9
+    sample = (f"each step = {n_sub}x{n_sub} strided sub-grid ({rays} rays) of the {args.n}x{args.n} image plane; "
+              f"ns/photon/step does not depend on the sampling density")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": tot_t / args.steps * 1e3,
+            "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": workload_name(args.n, args.a), "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------
+# the B200 arm
+# ---------------------------------------------------------------------------------------------------
+def run_b200(args):
+    import torch
+    import paper_1601_02063_b200 as ody
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the Odyssey hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    ody.load_library()
+    # Rays are independent: ranks share nothing; each rank renders one whole image per
+    # step (weak scaling, no data-path collective — DESIGN.md §9).
+    w = W.C4(n=args.n, a=args.a)
+    sc, mo, nu = w["scene"], w["model"], w["nu"][0]
+    out = ody.render_image(sc, mo, nu)
+    torch.cuda.synchronize()
+    for _ in range(max(args.warmup - 1, 0)):
+        ody.render_image(sc, mo, nu, out=out)
+    barrier()
+
+    # ---- timed region: exactly K steps, CUDA events on the launching (current) stream
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    launches0 = ody.launch_count()
+    barrier()
+    ev[0].record()
+    for k in range(args.steps):
+        ody.render_image(sc, mo, nu, out=out)
+        ev[k + 1].record()
+    barrier()
+    launches = ody.launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+    step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    total_ms = ev[0].elapsed_time(ev[args.steps])
+    attempts = int(out["n_attempt"].sum(dtype=torch.int64).item())
+    accepts = int(out["n_accept"].sum(dtype=torch.int64).item())
+    rays = sc["nx"] * sc["ny"]
+    out_bytes = sum(v.numel() * v.element_size() for v in out.values() if v is not None)
+
+    # ---- DFMA peak, same run, same clocks regime (burst figure: the probe is timed alone)
+    sink = torch.zeros(8, dtype=torch.float64, device="cuda")
+    ody.fp64_peak_probe(2000, sink)
+    torch.cuda.synchronize()
+    best = None
+    for _ in range(5):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        flop = ody.fp64_peak_probe(20000, sink)
+        e1.record()
+        torch.cuda.synchronize()
+        tf = flop / (e0.elapsed_time(e1) * 1e-3) / 1e12
+        best = tf if best is None else max(best, tf)
+    peak_tflops = best
+
+    # ---- end to end through the host-buffer C-ABI call (device alloc + kernel + D2H inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        host = ody.render_image_host(sc, mo, nu)                     # warm-up (also allocates the numpy buffers)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            ody.render_image_host(sc, mo, nu, out=host)
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        d2h = sum(v.nbytes for v in host.values() if v is not None)
+        h2d = 120 + 136 + 8                                           # the two structs and nu_hz (kernel parameters)
+        e2e = (e2e_s, d2h, h2d, int(host["n_attempt"].astype("int64").sum()))
+
+    # ---- reduce over ranks: time = max, work = sum
+    t = torch.tensor([total_ms, e2e[0] if e2e else 0.0], dtype=torch.float64, device="cuda")
+    n = torch.tensor([attempts, accepts, rays, launches], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    total_ms_max, e2e_s_max = t.tolist()
+    attempts_all, accepts_all, rays_all, launches_all = n.tolist()
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    ms_per_step = total_ms_max / args.steps
+    value = ms_per_step * 1e6 / attempts_all                          # ns per photon per attempted RK step
+    flop_step = FLOP_PER_ATTEMPT_GEODESIC * attempts + FLOP_PER_RT_UPDATE * accepts     # per launch (this rank)
+    kernel_ms = sum(step_ms) / len(step_ms)
+    achieved = flop_step / (kernel_ms * 1e-3) / 1e12
+    info = ody.kernel_info(2, False, sc["tableau"])
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args.n, args.a), "photons_per_step": int(rays_all),
+                   "attempted_rk_steps_per_step": int(attempts_all), "accepted_rk_steps_per_step": int(accepts_all),
+                   "attempts_per_photon": attempts_all / rays_all,
+                   "l2": "no input arrays (rays are generated from the pixel index); the %d MB of per-step "
+                         "outputs exceed the 126 MB L2" % (out_bytes >> 20),
+                   "parallelism": "replicas" if world > 1 else "single GPU"},
+        "images_per_s": world / (ms_per_step * 1e-3),
+        "ns_per_photon_per_accepted_step": ms_per_step * 1e6 / accepts_all,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                     "frac": achieved / peak_tflops, "traffic": None,
+                     "kernel": "odyssey_kernel<KIND=2,TAB=0,SPEC=false>", "kernel_ms": kernel_ms,
+                     "flop_per_attempt": FLOP_PER_ATTEMPT_GEODESIC, "flop_per_rt_update": FLOP_PER_RT_UPDATE,
+                     "peak_source": "odyssey_fp64_peak_probe (DFMA microbenchmark) in this run, best of 5"},
+        "kernel_info": info,
+        "gpu_launches": int(launches_all),
+        "clocks": clocks,
+        "paper_context": "~1 ns per photon per RK step claimed on a GTX 780 Ti (FP64, geodesics only); "
+                         "its Table 1 gives 25732 ms / 1.578e9 steps = 16.3 ns at 1024^2",
+    }
+    if e2e:
+        _, d2h, h2d, att_host = e2e
+        line["e2e"] = {"value": e2e_s_max / args.steps * 1e9 / (att_host * world), "unit": UNIT,
+                       "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                       "ms_per_step": e2e_s_max / args.steps * 1e3,
+                       "api": "odyssey_render_image_host (pageable host buffers)"}
+    if not args.no_cpu_baseline:
+        from oracle import build as oracle_build
+        oracle_build.build()
+        line["cpu_baseline"] = cpu_baseline(w, args.cpu_sample)
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_b200(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -102,10 +102,12 @@ int odyssey_trace_geodesics(const odyssey_scene* scene,
  *     (hist is overwritten, not accumulated across calls).
  *   kind 2 (eqs. (30),(31),(37)-(39)): image = I_nu = nu^3 × invariant intensity (erg s^-1 cm^-2
  *     Hz^-1 sr^-1), aux0 = optical depth tau, aux1 = 0.
- *   kind 0: image = aux0 = aux1 = 0; flags and step counts as odyssey_trace_geodesics.           */
+ *   kind 0: image = aux0 = aux1 = 0; flags and step counts as odyssey_trace_geodesics.
+ * n_attempt / n_accept: attempted and accepted Runge–Kutta steps per ray (one radiative-transfer
+ * update is made per accepted step).                                               */
 int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model, double nu_hz,
                          double* image, double* aux0, double* aux1, int32_t* flag,
-                         int32_t* n_attempt, double* hist, void* cuda_stream);
+                         int32_t* n_attempt, int32_t* n_accept, double* hist, void* cuda_stream);
 
 /* nf <= 32 observed frequencies integrated simultaneously along each geodesic (kind 2 only;
  * BASELINE.json:configs[3]).  images[nf][ny][nx] = I_nu; nuLnu[nf] = 4π nu r_g^2 Δx Δy Σ_pixels I_nu
@@ -121,7 +123,7 @@ int odyssey_trace_geodesics_host(const odyssey_scene* scene,
                                  int32_t* n_attempt, int32_t* n_accept);
 int odyssey_render_image_host(const odyssey_scene* scene, const odyssey_model* model, double nu_hz,
                               double* image, double* aux0, double* aux1, int32_t* flag,
-                              int32_t* n_attempt, double* hist);
+                              int32_t* n_attempt, int32_t* n_accept, double* hist);
 int odyssey_render_spectrum_host(const odyssey_scene* scene, const odyssey_model* model,
                                  const double* nu_hz_host, int nf,
                                  double* images, double* nuLnu, int32_t* flag, int32_t* n_attempt);

@@ -224,10 +224,11 @@ def render_image(scene, model, nu_hz=0.0, idx=None):
     n, ii, jj = _pixels(scene, idx)
     nb = int(model.get("nbins", 0))
     out = dict(image=np.zeros(n), aux0=np.zeros(n), aux1=np.zeros(n), flag=np.zeros(n, np.int32),
-               n_attempt=np.zeros(n, np.int32), hist=np.zeros(nb) if nb > 0 else None)
+               n_attempt=np.zeros(n, np.int32), n_accept=np.zeros(n, np.int32),
+               hist=np.zeros(nb) if nb > 0 else None)
     lib().oracle_render_image(C.byref(make_scene(scene)), C.byref(make_model(model)), C.c_double(nu_hz), C.c_int(n),
                               _ip(ii), _ip(jj), _dp(out["image"]), _dp(out["aux0"]), _dp(out["aux1"]),
-                              _ip(out["flag"]), _ip(out["n_attempt"]), _dp(out["hist"]))
+                              _ip(out["flag"]), _ip(out["n_attempt"]), _ip(out["n_accept"]), _dp(out["hist"]))
     return out
 
 

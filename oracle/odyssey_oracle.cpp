@@ -655,7 +655,8 @@ void oracle_trace_geodesics(const Scene* S, int n, const int32_t* idx_i, const i
 // (only when the whole grid is rendered).  kind 2: image = I_nu = nu^3 * invariant intensity (cgs),
 // aux0 = tau, aux1 = 0.
 void oracle_render_image(const Scene* S, const Model* M, double nu_hz, int n, const int32_t* idx_i, const int32_t* idx_j,
-                         double* image, double* aux0, double* aux1, int32_t* flag, int32_t* n_attempt, double* hist) {
+                         double* image, double* aux0, double* aux1, int32_t* flag, int32_t* n_attempt,
+                         int32_t* n_accept, double* hist) {
     int nf = (M->kind == 2) ? 1 : 0;
 #pragma omp parallel for schedule(dynamic, 16)
     for (int k = 0; k < n; ++k) {
@@ -667,6 +668,7 @@ void oracle_render_image(const Scene* S, const Model* M, double nu_hz, int n, co
         else if (M->kind == 2) { image[k] = nu_hz * nu_hz * nu_hz * R.I[0]; aux0[k] = R.tau[0]; aux1[k] = 0.0; }
         else { image[k] = 0.0; aux0[k] = 0.0; aux1[k] = 0.0; }
         flag[k] = R.flag; n_attempt[k] = R.n_attempt;
+        if (n_accept) n_accept[k] = R.n_accept;
     }
     if (hist && M->kind == 1 && M->nbins > 0) {       // serial, pixel order: line profile [reading Q]
         double area = ((S->x_max - S->x_min) / S->nx) * ((S->y_max - S->y_min) / S->ny);

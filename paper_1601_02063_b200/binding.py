@@ -74,11 +74,11 @@ def load_library():
         raise OdysseyError(f"cannot load {path}: {e}") from e
     vp, dp, ip = C.c_void_p, C.c_void_p, C.c_void_p
     L.odyssey_trace_geodesics.argtypes = [C.POINTER(Scene), ip, dp, dp, dp, ip, ip, vp]
-    L.odyssey_render_image.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.c_double, dp, dp, dp, ip, ip, dp, vp]
+    L.odyssey_render_image.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.c_double, dp, dp, dp, ip, ip, ip, dp, vp]
     L.odyssey_render_spectrum.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.POINTER(C.c_double), C.c_int,
                                           dp, dp, ip, ip, vp]
     L.odyssey_trace_geodesics_host.argtypes = [C.POINTER(Scene), ip, dp, dp, dp, ip, ip]
-    L.odyssey_render_image_host.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.c_double, dp, dp, dp, ip, ip, dp]
+    L.odyssey_render_image_host.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.c_double, dp, dp, dp, ip, ip, ip, dp]
     L.odyssey_render_spectrum_host.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.POINTER(C.c_double), C.c_int,
                                                dp, dp, ip, ip]
     L.odyssey_fp64_peak_probe.argtypes = [C.c_int, dp, C.POINTER(C.c_double), vp]
@@ -137,7 +137,7 @@ def trace_geodesics(scene):
 
 
 def render_image(scene, model, nu_hz=0.0, out=None):
-    """odyssey_render_image: image, aux0, aux1, flag, n_attempt ([ny, nx]) and hist ([nbins] or None).
+    """odyssey_render_image: image, aux0, aux1, flag, n_attempt, n_accept ([ny, nx]) and hist ([nbins] or None).
     `out` may carry pre-allocated tensors from a previous call (re-used, e.g. by bench.py)."""
     torch = _torch()
     L = load_library()
@@ -149,10 +149,12 @@ def render_image(scene, model, nu_hz=0.0, out=None):
                    aux1=torch.empty((ny, nx), **f64),
                    flag=torch.empty((ny, nx), dtype=torch.int32, device="cuda"),
                    n_attempt=torch.empty((ny, nx), dtype=torch.int32, device="cuda"),
+                   n_accept=torch.empty((ny, nx), dtype=torch.int32, device="cuda"),
                    hist=torch.empty((nb,), **f64) if nb > 0 else None)
     _check(L.odyssey_render_image(C.byref(_struct(Scene, scene)), C.byref(_struct(Model, model)), C.c_double(nu_hz),
                                   _ptr(out["image"]), _ptr(out["aux0"]), _ptr(out["aux1"]), _ptr(out["flag"]),
-                                  _ptr(out["n_attempt"]), _ptr(out.get("hist")), _stream(torch)))
+                                  _ptr(out["n_attempt"]), _ptr(out.get("n_accept")), _ptr(out.get("hist")),
+                                  _stream(torch)))
     return out
 
 
@@ -191,11 +193,11 @@ def render_image_host(scene, model, nu_hz=0.0, out=None):
         nb = int(model.get("nbins", 0)) if model["kind"] == 1 else 0
         out = dict(image=np.empty((ny, nx)), aux0=np.empty((ny, nx)), aux1=np.empty((ny, nx)),
                    flag=np.empty((ny, nx), np.int32), n_attempt=np.empty((ny, nx), np.int32),
-                   hist=np.empty(nb) if nb > 0 else None)
+                   n_accept=np.empty((ny, nx), np.int32), hist=np.empty(nb) if nb > 0 else None)
     _check(L.odyssey_render_image_host(C.byref(_struct(Scene, scene)), C.byref(_struct(Model, model)),
                                        C.c_double(nu_hz), _np_ptr(out["image"]), _np_ptr(out["aux0"]),
                                        _np_ptr(out["aux1"]), _np_ptr(out["flag"]), _np_ptr(out["n_attempt"]),
-                                       _np_ptr(out.get("hist"))))
+                                       _np_ptr(out.get("n_accept")), _np_ptr(out.get("hist"))))
     return out
 
 

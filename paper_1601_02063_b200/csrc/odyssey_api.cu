@@ -240,7 +240,7 @@ int odyssey_trace_geodesics(const odyssey_scene* scene, int32_t* flag, double* r
 
 int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model, double nu_hz,
                          double* image, double* aux0, double* aux1, int32_t* flag, int32_t* n_attempt,
-                         double* hist, void* cuda_stream) {
+                         int32_t* n_accept, double* hist, void* cuda_stream) {
     int rc = check_scene(scene);
     if (rc) return rc;
     rc = check_model(model);
@@ -248,7 +248,7 @@ int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model,
     if (model->kind == ODYSSEY_KIND_RIAF && !(nu_hz > 0.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz = %g must be > 0", nu_hz);
     Params P; fill_params(*scene, model, &nu_hz, 1, &P);
     Outputs O = no_outputs();
-    O.image = image; O.aux0 = aux0; O.aux1 = aux1; O.flag = flag; O.n_attempt = n_attempt;
+    O.image = image; O.aux0 = aux0; O.aux1 = aux1; O.flag = flag; O.n_attempt = n_attempt; O.n_accept = n_accept;
     O.hist = (model->kind == ODYSSEY_KIND_THIN_DISK && model->nbins > 0) ? hist : nullptr;
     return launch(P, O, false, scene->tableau, (cudaStream_t)cuda_stream);
 }
@@ -284,14 +284,15 @@ int odyssey_trace_geodesics_host(const odyssey_scene* scene, int32_t* flag, doub
 }
 
 int odyssey_render_image_host(const odyssey_scene* scene, const odyssey_model* model, double nu_hz,
-                              double* image, double* aux0, double* aux1, int32_t* flag, int32_t* n_attempt, double* hist) {
+                              double* image, double* aux0, double* aux1, int32_t* flag, int32_t* n_attempt,
+                              int32_t* n_accept, double* hist) {
     TRY(check_scene(scene)); TRY(check_model(model));
     const size_t n = (size_t)scene->nx * scene->ny;
-    Scratch S; double *dimg, *da0, *da1, *dhist; int32_t *dflag, *datt;
+    Scratch S; double *dimg, *da0, *da1, *dhist; int32_t *dflag, *datt, *dacc;
     TRY(S.add(image, n, &dimg)); TRY(S.add(aux0, n, &da0)); TRY(S.add(aux1, n, &da1));
-    TRY(S.add(flag, n, &dflag)); TRY(S.add(n_attempt, n, &datt));
+    TRY(S.add(flag, n, &dflag)); TRY(S.add(n_attempt, n, &datt)); TRY(S.add(n_accept, n, &dacc));
     TRY(S.add((model->kind == ODYSSEY_KIND_THIN_DISK && model->nbins > 0) ? hist : nullptr, (size_t)model->nbins, &dhist));
-    TRY(odyssey_render_image(scene, model, nu_hz, dimg, da0, da1, dflag, datt, dhist, nullptr));
+    TRY(odyssey_render_image(scene, model, nu_hz, dimg, da0, da1, dflag, datt, dacc, dhist, nullptr));
     return S.copy_back();
 }
 
