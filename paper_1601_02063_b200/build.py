@@ -9,6 +9,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libodyssey.so")
 SOURCES = ["odyssey_api.cu"]
 DEPS = ["odyssey_api.cu", "odyssey_kernels.cuh", "geodesic.cuh", "emission.cuh", "params.h", "bessel_k2_coeffs.h",
+        "dmath.cuh", "dmath_coeffs.h",
         os.path.join("..", "..", "include", "odyssey.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]

@@ -1,0 +1,183 @@
+// dmath.cuh — branch-free FP64 elementary functions for the Odyssey kernels.
+//
+// The CUDA math library's double-precision 1/x, sqrt, sincos, exp, log, expm1 each carry a slow path
+// (denormals, huge arguments) behind a branch.  In the fused geodesic + radiative-transfer loop those
+// branches (a) split the code into small basic blocks, so the scheduler cannot interleave the
+// independent dependency chains of one right-hand-side evaluation, and (b) add code that has to live
+// in the instruction cache.  The arguments on the hot path are all of ordinary magnitude (radii,
+// angles of a few radians, optical depths, exponents clamped to +-700), so the versions below do the
+// fast path only, straight-line:
+//
+//   d_rcp, d_rsqrt, d_sqrt : hardware seed (MUFU.RCP64H / MUFU.RSQ64H) + Newton steps in FMA
+//   d_sincos               : two-term Cody–Waite reduction by pi/2, odd/even polynomials on [-pi/4, pi/4]
+//   d_exp, d_expm1         : x = k ln2 + r, e^r = 1 + r q(r), scaling through the exponent field
+//   d_log                  : x = 2^e m, m in [sqrt(1/2), sqrt(2)), log m = 2 atanh((m-1)/(m+1))
+//
+// Accuracy: a few ulp (tests/test_dmath.py compares against libm on the host build of this header and
+// tests/test_gpu_dmath.py on the device).  Polynomial tables: dmath_coeffs.h (gen_dmath_coeffs.py).
+#pragma once
+#include <stdint.h>
+#include "dmath_coeffs.h"
+
+#if defined(__CUDACC__)
+#define ODY_HD __host__ __device__ __forceinline__
+#else
+#define ODY_HD inline
+#endif
+
+namespace ody {
+
+ODY_HD double d_from_bits(uint64_t u) {
+#if defined(__CUDA_ARCH__)
+    return __longlong_as_double((long long)u);
+#else
+    double d; __builtin_memcpy(&d, &u, 8); return d;
+#endif
+}
+ODY_HD uint64_t d_to_bits(double d) {
+#if defined(__CUDA_ARCH__)
+    return (uint64_t)__double_as_longlong(d);
+#else
+    uint64_t u; __builtin_memcpy(&u, &d, 8); return u;
+#endif
+}
+ODY_HD double d_fma(double a, double b, double c) {
+#if defined(__CUDA_ARCH__)
+    return fma(a, b, c);
+#else
+    return __builtin_fma(a, b, c);
+#endif
+}
+
+// ---- hardware seeds (about 20 good bits); the host versions exist only for the CPU unit test
+ODY_HD double d_rcp_seed(double x) {
+#if defined(__CUDA_ARCH__)
+    double y; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y;
+#else
+    return d_from_bits(d_to_bits(1.0 / x) & 0xfffffff000000000ull);
+#endif
+}
+ODY_HD double d_rsqrt_seed(double x) {
+#if defined(__CUDA_ARCH__)
+    double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y;
+#else
+    return d_from_bits(d_to_bits(1.0 / __builtin_sqrt(x)) & 0xfffffff000000000ull);
+#endif
+}
+
+// 1/x for normal x (no zero, infinity, NaN or denormal handling).
+ODY_HD double d_rcp(double x) {
+    double y = d_rcp_seed(x);
+    double e = d_fma(-x, y, 1.0);
+    e = d_fma(e, e, e);                 // e + e^2
+    y = d_fma(y, e, y);                 // third-order step
+    e = d_fma(-x, y, 1.0);
+    return d_fma(y, e, y);
+}
+
+// x^-1/2 for normal x > 0.
+ODY_HD double d_rsqrt(double x) {
+    double y = d_rsqrt_seed(x);
+    double e = d_fma(-x, y * y, 1.0);                 // 1 - x y^2
+    y = d_fma(y * e, d_fma(e, 0.375, 0.5), y);        // y (1 + e/2 + 3 e^2/8)
+    e = d_fma(-x, y * y, 1.0);
+    return d_fma(y * e, 0.5, y);
+}
+
+// sqrt(x) for normal x > 0 (x = 0 gives NaN: callers guard).
+ODY_HD double d_sqrt(double x) {
+    const double y = d_rsqrt(x);
+    const double s = x * y;
+    return d_fma(d_fma(-s, s, x), 0.5 * y, s);
+}
+
+#define ODY_COEF(i, v) v,
+
+// sin and cos of an angle of ordinary size (|x| < ~1e5; accuracy degrades slowly beyond).
+ODY_HD void d_sincos(double x, double& sn, double& cs) {
+    const double S[ODY_SINS_N] = { ODY_SINS(ODY_COEF) };
+    const double C[ODY_COSC_N] = { ODY_COSC(ODY_COEF) };
+    const double MAGIC = 6755399441055744.0;                       // 1.5 * 2^52: round-to-nearest-integer trick
+    const double t = d_fma(x, 0.63661977236758134308, MAGIC);      // x * 2/pi
+    const int32_t q = (int32_t)(uint32_t)d_to_bits(t);             // low word = nearest integer
+    const double k = t - MAGIC;
+    double r = d_fma(-k, 1.57079632679489655800e+00, x);           // pi/2 high part
+    r = d_fma(-k, 6.12323399573676603587e-17, r);                  // pi/2 low part
+    const double z = r * r;
+    double ps = S[ODY_SINS_N - 1], pc = C[ODY_COSC_N - 1];
+#if defined(__CUDA_ARCH__)
+#pragma unroll
+#endif
+    for (int i = ODY_SINS_N - 2; i >= 0; --i) { ps = d_fma(ps, z, S[i]); pc = d_fma(pc, z, C[i]); }
+    const double sr = d_fma(ps * z, r, r);                         // r + r^3 S(z)
+    const double cr = d_fma(z * z, pc, d_fma(-0.5, z, 1.0));       // 1 - z/2 + z^2 C(z)
+    const bool swap = q & 1;
+    double s0 = swap ? cr : sr, c0 = swap ? sr : cr;
+    if (q & 2) s0 = -s0;
+    if ((q + 1) & 2) c0 = -c0;
+    sn = s0; cs = c0;
+}
+
+// x = k ln2 + r with |r| <= ln2/2; returns r and 2^k (as a double), for |x| <= ~700.
+ODY_HD double d_exp_reduce(double x, double& two_k) {
+    const double MAGIC = 6755399441055744.0;
+    const double t = d_fma(x, 1.44269504088896338700e+00, MAGIC);
+    const int32_t k = (int32_t)(uint32_t)d_to_bits(t);
+    const double kf = t - MAGIC;
+    double r = d_fma(-kf, 6.93147180559945286227e-01, x);
+    r = d_fma(-kf, 2.31904681384629955842e-17, r);
+    two_k = d_from_bits((uint64_t)(uint32_t)(k + 1023) << 52);
+    return r;
+}
+
+ODY_HD double d_expq(double r) {                                   // (e^r - 1)/r
+    const double Q[ODY_EXPQ_N] = { ODY_EXPQ(ODY_COEF) };
+    double p = Q[ODY_EXPQ_N - 1];
+#if defined(__CUDA_ARCH__)
+#pragma unroll
+#endif
+    for (int i = ODY_EXPQ_N - 2; i >= 0; --i) p = d_fma(p, r, Q[i]);
+    return p;
+}
+
+// e^x; arguments below -700 return 0, above 700 are clamped (callers never get there with finite results).
+ODY_HD double d_exp(double x) {
+    const double xc = x < -700.0 ? -700.0 : (x > 700.0 ? 700.0 : x);
+    double two_k;
+    const double r = d_exp_reduce(xc, two_k);
+    const double v = d_fma(r * d_expq(r), two_k, two_k);           // 2^k (1 + r q)
+    return x < -700.0 ? 0.0 : v;
+}
+
+// e^x - 1, accurate near 0; same argument range as d_exp.
+ODY_HD double d_expm1(double x) {
+    const double xc = x < -700.0 ? -700.0 : (x > 700.0 ? 700.0 : x);
+    double two_k;
+    const double r = d_exp_reduce(xc, two_k);
+    return d_fma(r * d_expq(r), two_k, two_k - 1.0);               // 2^k r q + (2^k - 1)
+}
+
+// natural logarithm of a normal x > 0.
+ODY_HD double d_log(double x) {
+    const double P[ODY_LOGP_N] = { ODY_LOGP(ODY_COEF) };
+    const uint64_t u = d_to_bits(x);
+    // exponent chosen so that the mantissa m lies in [sqrt(1/2), sqrt(2)): add (1 - sqrt(1/2)) in the mantissa field
+    const uint64_t adj = u + 0x00095f619980c433ull;                // bits(1.0) - bits(sqrt(1/2))
+    const int32_t e = (int32_t)(adj >> 52) - 1023;
+    const double m = d_from_bits(u - ((uint64_t)(int64_t)e << 52));
+    const double f = m - 1.0;
+    const double s = f * d_rcp(2.0 + f);
+    const double z = s * s;
+    double p = P[ODY_LOGP_N - 1];
+#if defined(__CUDA_ARCH__)
+#pragma unroll
+#endif
+    for (int i = ODY_LOGP_N - 2; i >= 0; --i) p = d_fma(p, z, P[i]);
+    const double ef = (double)e;
+    // log x = e ln2 + 2 s p(z), ln2 split so that e * ln2_hi is exact
+    return d_fma(ef, 6.93147180369123816490e-01, d_fma(2.0 * s, p, ef * 1.90821492927058770002e-10));
+}
+
+#undef ODY_COEF
+
+}  // namespace ody

@@ -1,70 +1,91 @@
 // emission.cuh — device-side flow, energy shift and thermal-synchrotron coefficients.
 //
-//   flow_gamma     : flow four-velocity (Keplerian shells with u^θ = 0 outside the ISCO, PAPER.md:L268;
-//                    plunging with the ISCO's E, L inside, BASELINE.json:configs[2]) and the
-//                    energy-shift factor γ of eq. (2).
-//   bessel_k2      : K_2(x) of eq. (37); tables from gen_bessel_k2.py.
-//   rt_point       : plasma state (BASELINE.json:configs[2]) and what every frequency shares.
+//   flow_igamma    : flow four-velocity (Keplerian shells with u^θ = 0 outside the ISCO, PAPER.md:L268;
+//                    plunging with the ISCO's E, L inside, BASELINE.json:configs[2]) and 1/γ, γ the
+//                    energy-shift factor of eq. (2).
+//   bessel_k2_inv  : 1/K_2(x) of eq. (37) as (factor, exponent); tables from gen_bessel_k2.py.
+//   rt_point       : plasma state (BASELINE.json:configs[2]) and everything the frequencies share.
 //   rt_coefficients: per-frequency a = r_g α_0(ν_0)/γ and ε = r_g j_0(ν_0)/(γ ν_0³) of eqs. (30), (31)
 //                    with eqs. (37)-(39) and Kirchhoff's law.
 //   rt_update      : one accepted step of eqs. (30), (31) (reading E).
+//
+// Arithmetic layout.  Every factor of ε is a power law or an exponential, so the
+// product is assembled in log space and exponentiated ONCE per frequency:
+//   ε = r_g j_coef ν_0 n_e M(x_M) / (K_2(1/Θ_e) γ ν_0³)
+//     = r_g · Kfac · u² (1 + 0.40 u³ + 0.5316 u⁶) · exp( E + c_k − 1.8899 t⁴ ),
+//   t = x_M^(1/12) = exp((ln ν_k + ln(1/γ) − ln ν_c)/12),  u = 1/t,   (eq. (38): x^1/6 = t², x^1/4 = t³, x^1/3 = t⁴)
+//   E = ln(4.0505 j_coef) + ln n_e + Kexp − ln(1/γ),  c_k = −2 ln ν_k,  1/K_2 = Kfac · e^Kexp,
+//   a = ε · expm1(h ν_0 / k T_e) · c²/(2h)                              (Kirchhoff with B_ν0(T_e)),
+// with ln n_e, ln Θ_e, ln ν_c linear in ln r, cos²θ and constants.  Per point this needs two logarithms
+// (ln r, ln 1/γ) and one exponential (1/Θ_e); per frequency two exponentials and one expm1, instead of
+// the dozen pow/exp/cbrt/sqrt/divisions of the formulas as printed.  Same mathematics, different
+// rounding (parity tolerance on images: 1e-6 relative L1).
 #pragma once
 #include "params.h"
+#include "dmath.cuh"
 #include "bessel_k2_coeffs.h"
 
 namespace ody {
 
-// γ = 1/(u^t + p_r u^r + L u^φ) for k_t = −E = 1 (eq. (2) with a static observer at infinity).
+// 1/γ = u^t + p_r u^r + L u^φ for k_t = −E = 1 (eq. (2) with a static observer at infinity).
 // s, c = sinθ, cosθ.  Returns false where the flow has no normalisable velocity.
-__device__ __forceinline__ bool flow_gamma(const Params& P, const double L, const double r, const double s, const double c,
-                                           const double pr, double& gam) {
+__device__ __forceinline__ bool flow_igamma(const Params& P, const double L, const double r, const double s, const double c,
+                                            const double pr, double& igam) {
     const double a = P.a, a2 = P.a2;
     const double s2 = s * s, r2 = r * r;
     const double Sigma = fma(a2, c * c, r2);
     const double Delta = fma(r, r - 2.0, a2);
-    const double iS = 1.0 / Sigma;
+    const double iS = d_rcp(Sigma);
     // covariant metric, eq. (1)
     const double g_tt = -(1.0 - 2.0 * r * iS);
     const double g_tp = -2.0 * a * r * s2 * iS;
     const double g_pp = (r2 + a2 + 2.0 * a2 * r * s2 * iS) * s2;
     double Omega, ur = 0.0, ur2_grr = 0.0;
     if (r >= P.r_isco) {
-        Omega = 1.0 / fma(r, sqrt(r), a);
+        Omega = d_rcp(fma(r, d_sqrt(r), a));
     } else {
-        const double E = P.E_isco, Lk = P.L_isco, ir = 1.0 / r;
+        const double E = P.E_isco, Lk = P.L_isco, ir = d_rcp(r);
         const double ut_eq = (r2 + a2 + 2.0 * a2 * ir) * E - 2.0 * a * ir * Lk;      // × 1/Δ, cancels in Ω
         const double up_eq = 2.0 * a * ir * E + (1.0 - 2.0 * ir) * Lk;
-        Omega = up_eq / ut_eq;
+        Omega = up_eq * d_rcp(ut_eq);
         const double dl = Lk - a * E;
         double ur2 = E * E - 1.0 + 2.0 * ir - (Lk * Lk - a2 * (E * E - 1.0)) * ir * ir + 2.0 * dl * dl * ir * ir * ir;
-        if (ur2 < 0.0) ur2 = 0.0;
-        ur = -sqrt(ur2);
-        ur2_grr = ur2 * Sigma / Delta;                                            // g_rr (u^r)²
+        if (ur2 > 0.0) {
+            ur = -d_sqrt(ur2);
+            ur2_grr = ur2 * Sigma * d_rcp(Delta);                                 // g_rr (u^r)²
+        }
     }
     const double N = -(g_tt + 2.0 * Omega * g_tp + Omega * Omega * g_pp);
     if (!(N > 0.0)) return false;
-    const double ut = sqrt((1.0 + ur2_grr) / N);
-    gam = 1.0 / (ut + pr * ur + L * Omega * ut);
+    const double ut = d_sqrt(1.0 + ur2_grr) * d_rsqrt(N);
+    igam = fma(ut, fma(L, Omega, 1.0), pr * ur);
     return true;
 }
 
 #define ODY_X(i, v) v,
-__device__ __forceinline__ double bessel_k2(const double x) {
+// 1/K_2(x) = kfac · exp(kexp) for 0 < x; lx = ln x.
+__device__ __forceinline__ void bessel_k2_inv(const double x, const double lx, double& kfac, double& kexp) {
     if (x <= 2.0) {
         const double ca[ODY_K2_NS] = { ODY_K2_A(ODY_X) };
         const double cb[ODY_K2_NS] = { ODY_K2_B(ODY_X) };
         const double t = 0.25 * x * x;
+        const double lg = lx - 0.69314718055994530942;               // ln(x/2)
         double A = 0.0, B = 0.0;
 #pragma unroll
         for (int k = ODY_K2_NS - 1; k >= 0; --k) { A = fma(A, t, ca[k]); B = fma(B, t, cb[k]); }
-        return 2.0 / (x * x) - 0.5 + t * (B - log(0.5 * x) * A);
+        // x² K_2 = 2 − 2t + 4t² (B − ln(x/2) A)
+        const double S = fma(4.0 * t * t, fma(-lg, A, B), fma(-2.0, t, 2.0));
+        kfac = d_rcp(S);
+        kexp = 2.0 * lx;
     } else {
         const double cp[ODY_K2_NC + 1] = { ODY_K2_P(ODY_X) };
-        const double z = 4.0 / x - 1.0;
+        const double z = fma(4.0, d_rcp(x), -1.0);
         double F = 0.0;
 #pragma unroll
         for (int k = ODY_K2_NC; k >= 0; --k) F = fma(F, z, cp[k]);
-        return sqrt(1.5707963267948966 / x) * exp(-x) * F;
+        // K_2 = sqrt(π/2x) e^−x F(z)
+        kfac = d_rcp(F);
+        kexp = x + fma(0.5, lx, -0.22579135264472743236);            // ½ ln(2/π) = −0.2257913526…
     }
 }
 #undef ODY_X
@@ -72,51 +93,52 @@ __device__ __forceinline__ double bessel_k2(const double x) {
 // What all frequencies share at one point of the ray.
 struct RtPoint {
     bool on;            // inside the emitting region with a valid flow
-    double gam;         // γ
-    double n_e, T_e;    // cm^-3, K
-    double nu_c;        // eq. (39)
-    double jK;          // j_coef n_e / K_2(1/Θ_e)   (0 when K_2 underflows)
+    double fac;         // r_g · Kfac
+    double E;           // exponent shared by all frequencies
+    double lxm0;        // ln x_M − ln ν = ln(1/γ) − ln ν_c
+    double ycoef;       // h ν_0 /(k T_e) = ν · ycoef
 };
 
 __device__ __forceinline__ void rt_point(const Params& P, const double L, const double r, const double s, const double c,
                                          const double pr, RtPoint& q) {
     q.on = false;
     if (!(r > P.r_cap && r < P.r_rt_out)) return;
-    double gam;
-    if (!flow_gamma(P, L, r, s, c, pr, gam)) return;
-    if (!(gam > 0.0) || isinf(gam)) return;
-    const double lx = log(r / P.r_h);
-    const double n_e = P.n0 * exp(fma(P.n_index, lx, -c * c * P.inv_2h2));
-    const double T_e = P.T0 * exp(P.T_index * lx);
-    const double B = sqrt(P.B2_coef * n_e / r);
-    const double Theta = P.theta_per_K * T_e;
-    const double K2 = bessel_k2(1.0 / Theta);
-    q.on = true; q.gam = gam; q.n_e = n_e; q.T_e = T_e;
-    q.nu_c = P.nuc_coef * B * Theta * Theta;
-    q.jK = (K2 > 0.0) ? P.j_coef * n_e / K2 : 0.0;
+    double igam;
+    if (!flow_igamma(P, L, r, s, c, pr, igam)) return;
+    if (!(igam > 0.0) || isinf(igam)) return;
+    const double lr = d_log(r);
+    const double lrel = lr - P.ln_rh;                               // ln(r / r_h)
+    const double ln_ne = fma(P.n_index, lrel, fma(-c * c, P.inv_2h2, P.ln_n0));
+    const double ln_Th = fma(P.T_index, lrel, P.ln_Theta0);         // ln Θ_e
+    if (!(ln_Th > -6.5)) return;                                    // 1/Θ_e > 665: K_2 underflows, no emission
+    const double x = d_exp(-ln_Th);                                 // 1/Θ_e
+    double kfac, kexp;
+    bessel_k2_inv(x, -ln_Th, kfac, kexp);
+    const double ligam = d_log(igam);
+    // ln ν_c = ln nuc_coef + ½ (ln B2_coef + ln n_e − ln r) + 2 ln Θ_e         (eq. (39), B² = B2_coef n_e / r)
+    const double ln_nuc = fma(0.5, ln_ne - lr, fma(2.0, ln_Th, P.ln_nuc0));
+    q.on = true;
+    q.fac = P.rg_cm * kfac;
+    q.E = P.ln_j0 + ln_ne + kexp - ligam;
+    q.lxm0 = ligam - ln_nuc;
+    q.ycoef = P.h_over_mc2 * igam * x;
 }
 
-// eq. (38)
-__device__ __forceinline__ double mahadevan_M(const double xM) {
-    const double sq = sqrt(xM);          // x^1/2
-    const double qq = sqrt(sq);          // x^1/4
-    const double cb = cbrt(xM);          // x^1/3
-    const double sx = sqrt(cb);          // x^1/6
-    return 4.0505 / sx * (1.0 + 0.40 / qq + 0.5316 / sq) * exp(-1.8899 * cb);
-}
-
-__device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& q, const double nu, double& acoef, double& ecoef) {
+// Per-frequency coefficients.  ln_nu = ln ν_k.
+__device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& q, const double nu, const double ln_nu,
+                                                double& acoef, double& ecoef) {
     acoef = 0.0; ecoef = 0.0;
     if (!q.on) return;
-    const double igam = 1.0 / q.gam;
-    const double nu0 = nu * igam;                                   // local frequency (reading D)
-    const double Mx = mahadevan_M(nu0 / q.nu_c);
-    const double j = (Mx > 0.0) ? q.jK * nu0 * Mx : 0.0;            // eq. (37) per steradian (reading F)
-    const double nu03 = nu0 * nu0 * nu0;
-    const double Bnu = P.planck_coef * nu03 / expm1(P.h_over_k * nu0 / q.T_e);
-    const double alpha = (j > 0.0 && Bnu > 0.0) ? j / Bnu : 0.0;    // Kirchhoff
-    acoef = P.rg_cm * alpha * igam;
-    ecoef = P.rg_cm * j * igam / nu03;
+    const double t = d_exp((ln_nu + q.lxm0) * (1.0 / 12.0));        // x_M^(1/12)
+    const double u = d_rcp(t);
+    const double t2 = t * t, u2 = u * u;
+    const double u3 = u2 * u;
+    const double poly = fma(u3, fma(0.5316, u3, 0.40), 1.0);        // eq. (38) bracket
+    const double ex = d_exp(fma(-1.8899, t2 * t2, fma(-2.0, ln_nu, q.E)));
+    const double eps = q.fac * u2 * poly * ex;                       // reading D, F
+    const double em1 = d_expm1(nu * q.ycoef);                        // e^{hν0/kT} − 1
+    ecoef = eps;
+    acoef = (eps > 0.0 && nu * q.ycoef < 700.0) ? eps * em1 * P.inv_planck : 0.0;   // Kirchhoff
 }
 
 // Trapezoid in λ for Δτ and the emission, exact attenuation across the step: φ(x) = (1 − e^−x)/x.
@@ -124,10 +146,10 @@ __device__ __forceinline__ void rt_update(const double a0, const double a1, cons
                                           const double dl, const double tau_max, double& tau, double& T, double& I) {
     if (tau > tau_max) return;
     const double dtau = 0.5 * (a0 + a1) * dl;
-    const double em = expm1(-dtau);                                 // e^−Δτ − 1
-    const double phi = (dtau > 0.0) ? -em / dtau : 1.0;
+    const double em = d_expm1(-dtau);                                // e^−Δτ − 1
+    const double phi = (dtau > 1e-300) ? -em * d_rcp(dtau) : 1.0;
     I = fma(T * (0.5 * (e0 + e1) * dl), phi, I);
-    T *= (1.0 + em);
+    T = fma(T, em, T);
     tau += dtau;
 }
 

@@ -5,7 +5,7 @@
 //   geodesic_rhs  : the five right-hand sides, eqs. (4), (5), (12) and -dH/dr, -dH/dθ of the
 //                   un-substituted Hamiltonian (≡ eqs. (14), (15) on the null shell; DESIGN.md
 //                   reading A), pole clamp of PAPER.md:L90.
-//   rk_stages     : stages 2..6 of an embedded 6-stage Runge–Kutta 5(4) pair ("fifth-
+//   stage_point / rk_combine : stages 2..6 of an embedded 6-stage Runge–Kutta 5(4) pair ("fifth-
 //                   order Runge–Kutta … adaptive step size", Press et al. 1992) with the first
 //                   slope k1 supplied by the caller (it is cached across rejected attempts).
 //
@@ -13,6 +13,7 @@
 // which is folded into the formulas below: P = (r²+a²)E − aL = −Pm with Pm = r² + a² + aL.
 #pragma once
 #include "params.h"
+#include "dmath.cuh"
 
 namespace ody {
 
@@ -26,14 +27,14 @@ __device__ __forceinline__ void geodesic_rhs(const double a, const double a2, co
                                              const double r, const double th, const double pr, const double pth,
                                              Slope& k, double& sin_th, double& cos_th) {
     double s, c;
-    sincos(th, &s, &c);
+    d_sincos(th, s, c);
     sin_th = s; cos_th = c;
     if (fabs(s) < 1e-8) s = copysign(1e-8, s);
     const double r2 = r * r;
     const double Sigma = fma(a2, c * c, r2);                      // Σ = r² + a² cos²θ
     const double Delta = fma(r, r - 2.0, a2);                     // Δ = r² − 2r + a²
     const double Pm = r2 + fma(a, L, a2);                         // −P
-    const double iS = 1.0 / Sigma, iD = 1.0 / Delta, is = 1.0 / s;
+    const double iS = d_rcp(Sigma), iD = d_rcp(Delta), is = d_rcp(s);   // three independent Newton chains
     const double is2 = is * is;
     const double D = fma(L, is, a * s);                           // L/sinθ − aE sinθ
     const double q = Pm * iD;                                     // −P/Δ
@@ -100,57 +101,74 @@ __host__ __device__ constexpr double rk_b4(int j) {
     }
 }
 
-// One attempt of size h from y with first slope k1: fifth-order result ynew and the error estimate
-// yerr = h Σ (b5_j − b4_j) k_j (as Press et al.'s rkck forms it).  φ does not enter the right-hand
-// side, so its stage values are never formed; only its two weighted sums are accumulated.
-template <int TAB>
-__device__ __forceinline__ void rk_attempt(const double a, const double a2, const double L,
-                                           const State& y, const Slope& k1, const double h,
-                                           State& ynew, State& yerr) {
-    double kr[6], kt[6], kp[6], kq[6];      // slopes of r, θ, p_r, p_θ per stage (registers after unrolling)
-    kr[0] = k1.r; kt[0] = k1.th; kp[0] = k1.pr; kq[0] = k1.pth;
-    double ph5 = rk_b5<TAB>(0) * k1.ph;
-    double phe = (rk_b5<TAB>(0) - rk_b4<TAB>(0)) * k1.ph;
+// The four dynamic components' slopes of the six stages (φ does not enter the right-hand side, so its
+// stage values are never formed; only its two weighted sums are accumulated by the kernel).
+// Two storage policies with the same interface:
+//   StagesReg  : 24 doubles in registers (spectrum kernel: one block per SM, registers to spare);
+//   StagesSmem : 24 doubles per thread in shared memory, [component][stage][thread] — consecutive lanes
+//                hit consecutive 8-byte words, so every access is conflict-free.  This takes 48
+//                registers off the main kernel, which is what lets it run 4 blocks of 128 threads per SM.
+struct StagesReg {
+    double v[4][6];
+    __device__ __forceinline__ double get(int c, int j) const { return v[c][j]; }
+    __device__ __forceinline__ void set(int c, int j, double x) { v[c][j] = x; }
+};
+template <int NT>
+struct StagesSmem {
+    double* base;                                       // &smem[threadIdx.x]
+    __device__ __forceinline__ double get(int c, int j) const { return base[(c * 6 + j) * NT]; }
+    __device__ __forceinline__ void set(int c, int j, double x) { base[(c * 6 + j) * NT] = x; }
+};
+
+// Argument of stage I+1 (0-based I in 1..5): y + h Σ_{j<I} a_Ij k_j.
+template <int TAB, int I, class KS>
+__device__ __forceinline__ void stage_point(const KS& K, const State& y, const double h,
+                                            double& r, double& th, double& pr, double& pth) {
+    double sr = 0.0, st = 0.0, sp = 0.0, sq = 0.0;
 #pragma unroll
-    for (int i = 1; i < 6; ++i) {
-        double sr = 0.0, st = 0.0, sp = 0.0, sq = 0.0;
-#pragma unroll
-        for (int j = 0; j < i; ++j) {
-            const double aij = rk_a<TAB>(i, j);
-            if (aij != 0.0) {
-                sr = fma(aij, kr[j], sr); st = fma(aij, kt[j], st);
-                sp = fma(aij, kp[j], sp); sq = fma(aij, kq[j], sq);
-            }
+    for (int j = 0; j < I; ++j) {
+        const double aij = rk_a<TAB>(I, j);
+        if (aij != 0.0) {
+            sr = fma(aij, K.get(0, j), sr); st = fma(aij, K.get(1, j), st);
+            sp = fma(aij, K.get(2, j), sp); sq = fma(aij, K.get(3, j), sq);
         }
-        Slope k; double s_, c_;
-        geodesic_rhs(a, a2, L, fma(h, sr, y.r), fma(h, st, y.th), fma(h, sp, y.pr), fma(h, sq, y.pth), k, s_, c_);
-        kr[i] = k.r; kt[i] = k.th; kp[i] = k.pr; kq[i] = k.pth;
-        const double b5 = rk_b5<TAB>(i), be = rk_b5<TAB>(i) - rk_b4<TAB>(i);
-        if (b5 != 0.0) ph5 = fma(b5, k.ph, ph5);
-        if (be != 0.0) phe = fma(be, k.ph, phe);
     }
-    double s5r = 0.0, s5t = 0.0, s5p = 0.0, s5q = 0.0, ser = 0.0, set = 0.0, sep = 0.0, seq = 0.0;
+    r = fma(h, sr, y.r); th = fma(h, st, y.th); pr = fma(h, sp, y.pr); pth = fma(h, sq, y.pth);
+}
+
+// Fifth-order result and the error estimate h Σ (b5_j − b4_j) k_j (as Press et al.'s rkck forms it)
+// of the four dynamic components; ph5 / phe are the kernel's running φ sums.
+template <int TAB, class KS>
+__device__ __forceinline__ void rk_combine(const KS& K, const State& y, const double h, const double ph5, const double phe,
+                                           State& ynew, State& yerr) {
+    double s5[4] = {0.0, 0.0, 0.0, 0.0}, se[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
         const double b5 = rk_b5<TAB>(j), be = rk_b5<TAB>(j) - rk_b4<TAB>(j);
-        if (b5 != 0.0) { s5r = fma(b5, kr[j], s5r); s5t = fma(b5, kt[j], s5t); s5p = fma(b5, kp[j], s5p); s5q = fma(b5, kq[j], s5q); }
-        if (be != 0.0) { ser = fma(be, kr[j], ser); set = fma(be, kt[j], set); sep = fma(be, kp[j], sep); seq = fma(be, kq[j], seq); }
+        if (b5 != 0.0 || be != 0.0) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const double k = K.get(c, j);
+                if (b5 != 0.0) s5[c] = fma(b5, k, s5[c]);
+                if (be != 0.0) se[c] = fma(be, k, se[c]);
+            }
+        }
     }
-    ynew.r = fma(h, s5r, y.r); ynew.th = fma(h, s5t, y.th); ynew.ph = fma(h, ph5, y.ph);
-    ynew.pr = fma(h, s5p, y.pr); ynew.pth = fma(h, s5q, y.pth);
-    yerr.r = h * ser; yerr.th = h * set; yerr.ph = h * phe; yerr.pr = h * sep; yerr.pth = h * seq;
+    ynew.r = fma(h, s5[0], y.r); ynew.th = fma(h, s5[1], y.th); ynew.ph = fma(h, ph5, y.ph);
+    ynew.pr = fma(h, s5[2], y.pr); ynew.pth = fma(h, s5[3], y.pth);
+    yerr.r = h * se[0]; yerr.th = h * se[1]; yerr.ph = h * phe; yerr.pr = h * se[2]; yerr.pth = h * se[3];
 }
 
 // Scaled max-norm of the error in units of rtol (reading G): scales (|r|, 1, 1, 1+|p_r|,
 // 1+|p_θ|).  A NaN anywhere yields NaN (the attempt is then rejected with h × 0.1).
-__device__ __forceinline__ double error_norm(const State& y, const State& e, const double rtol) {
-    const double q0 = fabs(e.r) / fabs(y.r);
+__device__ __forceinline__ double error_norm(const State& y, const State& e, const double inv_rtol) {
+    const double q0 = fabs(e.r) * d_rcp(fabs(y.r));
     const double q1 = fabs(e.th), q2 = fabs(e.ph);
-    const double q3 = fabs(e.pr) / (1.0 + fabs(y.pr));
-    const double q4 = fabs(e.pth) / (1.0 + fabs(y.pth));
+    const double q3 = fabs(e.pr) * d_rcp(1.0 + fabs(y.pr));
+    const double q4 = fabs(e.pth) * d_rcp(1.0 + fabs(y.pth));
     const double m = fmax(fmax(fmax(q0, q1), fmax(q2, q3)), q4);   // fmax drops NaNs …
     const double sum = q0 + q1 + q2 + q3 + q4;                     // … so detect them here (all q ≥ 0)
-    return (sum != sum) ? sum : m / rtol;
+    return (sum != sum) ? sum : m * inv_rtol;
 }
 
 // x^(-1/5) for x in (0, 1]: single-precision seed, two Newton steps y ← y (6 − x y⁵)/5 in FP64.

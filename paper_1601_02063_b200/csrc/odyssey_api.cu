@@ -95,8 +95,9 @@ int check_model(const odyssey_model* M) {
         if (M->nbins > 0 && !(M->g_hi > M->g_lo)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "g_hi must exceed g_lo");
     }
     if (M->kind == ODYSSEY_KIND_RIAF) {
-        if (!(M->mbh_msun > 0.0) || !(M->h_over_r > 0.0) || !(M->beta > 0.0) || !(M->T0 > 0.0) || !(M->n0 >= 0.0))
-            return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "RIAF parameters mbh_msun, h_over_r, beta, T0 must be positive");
+        if (!(M->mbh_msun > 0.0) || !(M->h_over_r > 0.0) || !(M->beta > 0.0) || !(M->T0 > 0.0) || !(M->n0 >= 0.0) ||
+            !(M->j_scale >= 0.0))
+            return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "RIAF parameters mbh_msun, h_over_r, beta, T0 must be positive, n0 and j_scale non-negative");
     }
     return ODYSSEY_OK;
 }
@@ -109,7 +110,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
     P->sin_pobs = std::sin(S.phi_obs); P->cos_pobs = std::cos(S.phi_obs); P->phi_obs = S.phi_obs;
     P->x_min = S.x_min; P->x_span = S.x_max - S.x_min; P->y_min = S.y_min; P->y_span = S.y_max - S.y_min;
     P->pix_area = (P->x_span / S.nx) * (P->y_span / S.ny);
-    P->rtol = S.rtol; P->h0 = S.h0;
+    P->rtol = S.rtol; P->inv_rtol = 1.0 / S.rtol; P->h0 = S.h0;
     P->r_h = 1.0 + std::sqrt(1.0 - S.a * S.a);
     P->r_cap = P->r_h + S.horizon_eps; P->r_esc = S.r_esc;
     P->nx = S.nx; P->ny = S.ny; P->max_attempts = S.max_attempts;
@@ -133,23 +134,24 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
         P->g_lo = M->g_lo; P->g_hi = M->g_hi; P->nbins = M->nbins;
     }
     if (M->kind == ODYSSEY_KIND_RIAF) {
-        P->n0 = M->n0; P->n_index = M->n_index; P->T0 = M->T0; P->T_index = M->T_index;
+        P->n_index = M->n_index; P->T_index = M->T_index;
         P->inv_2h2 = 1.0 / (2.0 * M->h_over_r * M->h_over_r);
-        P->B2_coef = 8.0 * kPi * kMp * kC * kC / (6.0 * M->beta);
-        P->theta_per_K = kKB / (kMe * kC * kC);
-        P->nuc_coef = 3.0 * kE / (4.0 * kPi * kMe * kC);
-        P->j_coef = M->j_scale * kE * kE / (std::sqrt(3.0) * kC);
-        P->planck_coef = 2.0 * kH / (kC * kC);
-        P->h_over_k = kH / kKB;
+        P->ln_rh = std::log(P->r_h);
+        P->ln_n0 = std::log(M->n0);                                   // -inf for n0 = 0: no emission
+        P->ln_Theta0 = std::log(kKB * M->T0 / (kMe * kC * kC));
+        P->ln_nuc0 = std::log(3.0 * kE / (4.0 * kPi * kMe * kC)) + 0.5 * std::log(8.0 * kPi * kMp * kC * kC / (6.0 * M->beta));
+        P->ln_j0 = std::log(4.0505 * M->j_scale * kE * kE / (std::sqrt(3.0) * kC));
+        P->h_over_mc2 = kH / (kMe * kC * kC);
+        P->inv_planck = kC * kC / (2.0 * kH);
         P->r_rt_out = M->r_rt_out; P->tau_max = M->tau_max;
         P->rg_cm = kGMsun * M->mbh_msun / (kC * kC);
         P->sed_coef = 4.0 * kPi * P->rg_cm * P->rg_cm * P->pix_area;
-        for (int k = 0; k < nf && k < MAX_FREQ; ++k) { P->nu[k] = nu[k]; P->nu3[k] = nu[k] * nu[k] * nu[k]; }
+        for (int k = 0; k < nf && k < MAX_FREQ; ++k) { P->nu[k] = nu[k]; P->ln_nu[k] = std::log(nu[k]); P->nu3[k] = nu[k] * nu[k] * nu[k]; }
     }
 }
 
 // ---- kernel table ------------------------------------------------------------------------------
-constexpr int NT_MAIN = 128, MINB_MAIN = 3;     // 168 registers per thread at most
+constexpr int NT_MAIN = 128, MINB_MAIN = 4;     // 128 registers per thread at most
 constexpr int NT_SPEC = 160, MINB_SPEC = 1;     // 5 x 32 x 160 x 8 B = 200 KiB of accumulators
 
 typedef void (*KernelFn)(const Params, const Outputs);
@@ -165,8 +167,9 @@ KernelFn pick_kernel(int kind, bool spec, int tab) {
 
 size_t smem_bytes(int kind, bool spec, int nf, int nbins) {
     if (spec) return (size_t)(5 * nf * NT_SPEC + MAX_FREQ) * sizeof(double);
-    if (kind == 1) return (size_t)(nbins > 0 ? nbins : 1) * sizeof(double);
-    return 0;
+    const size_t stages = (size_t)24 * NT_MAIN * sizeof(double);         // [4][6][NT] stage slopes
+    if (kind == 1) return stages + (size_t)(nbins > 0 ? nbins : 1) * sizeof(double);
+    return stages;
 }
 
 int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {

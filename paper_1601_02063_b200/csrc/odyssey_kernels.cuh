@@ -4,12 +4,19 @@
 // the kernel is PERSISTENT: every lane pulls its next pixel from an atomic work queue as soon as
 // its ray ends (horizon capture, escape, disk hit, optical-depth cutoff), so warps stay full.
 //
-// Lane life cycle (one trip round the main loop = one Runge–Kutta attempt for every live lane):
+// One trip round the main loop = one Runge–Kutta attempt for every live lane of the warp:
 //   refill  : lanes without a ray ballot; the leader takes popc(ballot) queue slots with ONE
 //             atomicAdd; slot q -> tile q/32 (8x4 pixels, row-major tiles) -> pixel; init_ray.
-//   attempt : stages 2..6 from (y, k1, h); the first slope k1 = f(y) is cached, so a rejected
-//             attempt or a re-attempt of the event location costs 5 right-hand sides, not 6.
-//   control : scaled max-norm error vs rtol; reject -> shrink h; accept -> h_next.
+//             A new lane is FRESH for this trip: it sits out stages 2..5 and uses the sixth
+//             right-hand-side slot to evaluate f(y0) (its first slope) and, in the transfer block,
+//             the absorption / emission coefficients at its start point.
+//   stages  : a real loop over the stage index s = 1..6 around ONE copy of the right-hand side
+//             (the instruction cache holds ~32 KB; six inlined copies of f plus the transfer code
+//             would not fit).  s is warp-uniform.  Stages 1..5 are the tableau's stages 2..6; slot 6
+//             forms the fifth-order result and the error estimate, takes the accept/reject decision
+//              and evaluates f at the accepted end state (next step's first
+//             slope, the Newton derivative of the event location, sinθ/cosθ for the transfer).
+//             The first slope k1 = f(y) is cached, so a rejected attempt costs 5 evaluations.
 //   events  : equatorial crossing (thin disk), capture, escape.  The event LOCATION (Newton on h,
 //             re-taking the step from y) is a lane MODE, not an inner loop: a locating lane simply
 //             makes its next attempt with the corrected h alongside its warp-mates' normal attempts.
@@ -20,13 +27,14 @@
 // accumulators in shared memory laid out [quantity][frequency][thread] (bank-conflict free).
 #pragma once
 #include <cuda_runtime.h>
+#include <type_traits>
 #include "params.h"
 #include "geodesic.cuh"
 #include "emission.cuh"
 
 namespace ody {
 
-constexpr int M_NORMAL = 0, M_EQ = 1, M_CAP = 2, M_ESC = 3;       // lane modes
+constexpr int M_NORMAL = 0, M_EQ = 1, M_CAP = 2, M_ESC = 3, M_FRESH = 4;       // lane modes
 constexpr int F_ESCAPED = 0, F_CAPTURED = 1, F_DISK = 2, F_OPAQUE = 3, F_MAXSTEP = 4;
 constexpr unsigned FULL = 0xffffffffu;
 constexpr double HALF_PI = 1.57079632679489661923;
@@ -38,15 +46,24 @@ __device__ __forceinline__ int radial_event(const Params& P, const State& yn) {
     return M_NORMAL;
 }
 
+template <int TAB, int I, class KS>
+__device__ __forceinline__ void store_stage(KS& K, const Slope& k, double& ph5, double& phe) {
+    K.set(0, I, k.r); K.set(1, I, k.th); K.set(2, I, k.pr); K.set(3, I, k.pth);
+    constexpr double b5 = rk_b5<TAB>(I), be = rk_b5<TAB>(I) - rk_b4<TAB>(I);
+    if (b5 != 0.0) ph5 = fma(b5, k.ph, ph5);
+    if (be != 0.0) phe = fma(be, k.ph, phe);
+}
+
 template <int KIND, int TAB, bool SPEC, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB)
 odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs O) {
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31;
     const int nf = SPEC ? P.nf : 1;
-    // shared layout: SPEC: [5][nf][NT] accumulators then sed[MAX_FREQ]; KIND 1: hist[nbins]
+    // shared layout: SPEC: [5][nf][NT] accumulators then sed[MAX_FREQ];
+    //                otherwise: [4][6][NT] stage slopes, then (KIND 1) hist[nbins]
     double* const sm_acc = smem;
-    double* const sm_red = SPEC ? smem + 5 * nf * NT : smem;
+    double* const sm_red = SPEC ? smem + 5 * nf * NT : smem + 24 * NT;
     if (SPEC) { for (int k = threadIdx.x; k < MAX_FREQ; k += NT) sm_red[k] = 0.0; }
     if (KIND == 1) { for (int k = threadIdx.x; k < P.nbins; k += NT) sm_red[k] = 0.0; }
     if (SPEC || KIND == 1) __syncthreads();
@@ -55,12 +72,16 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     const double a = P.a, a2 = P.a2;
     bool active = false, exhausted = false, on_eq = false;
     int pix = 0, n_att = 0, n_acc = 0, mode = M_NORMAL, loc_it = 0;
-    State y; Slope k1;
+    State y;
+    typename std::conditional<SPEC, StagesReg, StagesSmem<NT>>::type K;
+    if constexpr (!SPEC) K.base = smem + threadIdx.x;
+    double kph0 = 0.0;                                              // φ slope of the cached first stage
     double L = 0.0, h_try = 0.0, h_next = 0.0, cos_y = 0.0;
     double tau = 0.0, Tr = 1.0, Inu = 0.0, a0 = 0.0, e0 = 0.0;      // single-frequency RT state
     double g_disk = 0.0, r_e = 0.0;
     y.r = y.th = y.ph = y.pr = y.pth = 0.0;
-    k1.r = k1.th = k1.ph = k1.pr = k1.pth = 0.0;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) { K.set(0, j, 0.0); K.set(1, j, 0.0); K.set(2, j, 0.0); K.set(3, j, 0.0); }
 
     for (;;) {
         // ------------------------------------------------------------------ refill from the queue
@@ -82,22 +103,14 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                         const double x = P.x_min + (i + 0.5) * P.x_span / P.nx;      // pixel centres (reading K)
                         const double yy = P.y_min + (j + 0.5) * P.y_span / P.ny;
                         init_ray(P, x, yy, y, L);
-                        double s0, c0;
-                        geodesic_rhs(a, a2, L, y.r, y.th, y.pr, y.pth, k1, s0, c0);
-                        cos_y = c0;
                         pix = j * P.nx + i;
-                        n_att = 0; n_acc = 0; mode = M_NORMAL; loc_it = 0; on_eq = false;
-                        h_try = P.h0; g_disk = 0.0; r_e = 0.0;
+                        n_att = 0; n_acc = 0; mode = M_FRESH; loc_it = 0; on_eq = false;
+                        h_try = P.h0; h_next = P.h0; g_disk = 0.0; r_e = 0.0;
                         if (KIND == 2) {
-                            RtPoint pt; rt_point(P, L, y.r, s0, c0, y.pr, pt);
                             if (SPEC) {
-                                for (int k = 0; k < nf; ++k) {
-                                    double ac, ec; rt_coefficients(P, pt, P.nu[k], ac, ec);
-                                    ACC(0, k) = 0.0; ACC(1, k) = 1.0; ACC(2, k) = 0.0; ACC(3, k) = ac; ACC(4, k) = ec;
-                                }
+                                for (int k = 0; k < nf; ++k) { ACC(0, k) = 0.0; ACC(1, k) = 1.0; ACC(2, k) = 0.0; ACC(3, k) = 0.0; ACC(4, k) = 0.0; }
                             } else {
-                                rt_coefficients(P, pt, P.nu[0], a0, e0);
-                                tau = 0.0; Tr = 1.0; Inu = 0.0;
+                                tau = 0.0; Tr = 1.0; Inu = 0.0; a0 = 0.0; e0 = 0.0;
                             }
                         }
                         active = true;
@@ -109,31 +122,68 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             if (__all_sync(FULL, exhausted)) break;
             continue;
         }
-        if (!active) continue;
 
         // ------------------------------------------------------------------ one attempt
         int flag = -1;
-        if (mode == M_NORMAL && n_att >= P.max_attempts) {
-            flag = F_MAXSTEP;
-        } else {
-            State yn, ye;
-            rk_attempt<TAB>(a, a2, L, y, k1, h_try, yn, ye);
-            ++n_att;
-            if (mode == M_NORMAL) {
-                const double err = error_norm(y, ye, P.rtol);
-                if (!(err <= 1.0)) {                                   // reject (also NaN)
-                    h_try *= isfinite(err) ? fmax(0.1, 0.9 * rsqrt(sqrt(err))) : 0.1;
-                    continue;
-                }
-                ++n_acc;
-                h_next = h_try * ((err < 1.889568e-4) ? 5.0 : fmin(5.0, 0.9 * inv_fifth_root(err)));
-            } else {
-                ++loc_it;
-            }
-            // slopes at the candidate end state: next step's k1, the Newton derivative, sinθ/cosθ for the RT
-            Slope kn; double sn, cn;
-            geodesic_rhs(a, a2, L, yn.r, yn.th, yn.pr, yn.pth, kn, sn, cn);
+        const bool fresh = active && mode == M_FRESH;
+        bool run = active && !fresh;                                   // takes part in stages 2..6
+        if (run && mode == M_NORMAL && n_att >= P.max_attempts) { flag = F_MAXSTEP; run = false; }
+        bool done = false;                                             // end state evaluated: go on to events / commit
+        double ph5 = rk_b5<TAB>(0) * kph0;
+        double phe = (rk_b5<TAB>(0) - rk_b4<TAB>(0)) * kph0;
+        State yn; Slope kn; double sn, cn;                             // defined in slot 6, read only when `done`
 
+#pragma unroll 1
+        for (int s = 1; s <= 6; ++s) {
+            double ir = y.r, ith = y.th, ipr = y.pr, ipth = y.pth;
+            bool ev = run;
+            switch (s) {
+                case 1: stage_point<TAB, 1>(K, y, h_try, ir, ith, ipr, ipth); break;
+                case 2: stage_point<TAB, 2>(K, y, h_try, ir, ith, ipr, ipth); break;
+                case 3: stage_point<TAB, 3>(K, y, h_try, ir, ith, ipr, ipth); break;
+                case 4: stage_point<TAB, 4>(K, y, h_try, ir, ith, ipr, ipth); break;
+                case 5: stage_point<TAB, 5>(K, y, h_try, ir, ith, ipr, ipth); break;
+                default: {
+                    if (run) {
+                        State ye;
+                        rk_combine<TAB>(K, y, h_try, ph5, phe, yn, ye);
+                        ++n_att;
+                        if (mode == M_NORMAL) {
+                            const double err = error_norm(y, ye, P.inv_rtol);
+                            if (!(err <= 1.0)) {                       // reject (also NaN): shrink, keep k1
+                                h_try *= isfinite(err) ? fmax(0.1, 0.9 * d_rsqrt(d_sqrt(err))) : 0.1;
+                                ev = false;
+                            } else {
+                                ++n_acc;
+                                h_next = h_try * ((err < 1.889568e-4) ? 5.0 : fmin(5.0, 0.9 * inv_fifth_root(err)));
+                            }
+                        } else {
+                            ++loc_it;
+                        }
+                    }
+                    if (!run) yn = y;                                  // a fresh lane evaluates f(y0) here
+                    ev = ev || fresh;
+                    done = ev;
+                    ir = yn.r; ith = yn.th; ipr = yn.pr; ipth = yn.pth;
+                }
+            }
+            if (ev) {
+                Slope k; double s_, c_;
+                geodesic_rhs(a, a2, L, ir, ith, ipr, ipth, k, s_, c_);
+                switch (s) {
+                    case 1: store_stage<TAB, 1>(K, k, ph5, phe); break;
+                    case 2: store_stage<TAB, 2>(K, k, ph5, phe); break;
+                    case 3: store_stage<TAB, 3>(K, k, ph5, phe); break;
+                    case 4: store_stage<TAB, 4>(K, k, ph5, phe); break;
+                    case 5: store_stage<TAB, 5>(K, k, ph5, phe); break;
+                    default: kn = k; sn = s_; cn = c_;
+                }
+            }
+        }
+
+        // ------------------------------------------------------------------ events on the evaluated end state
+        bool commit = false;
+        if (done && !fresh) {
             if (mode == M_NORMAL) {                                    // fresh accepted step: detect events
                 int m = M_NORMAL;
                 if (KIND == 1) {
@@ -157,8 +207,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     on_eq = true; mode = M_NORMAL;
                     if (yn.r >= P.r_in && yn.r <= P.r_out && yn.r > P.r_cap) {
                         flag = F_DISK; r_e = yn.r;
-                        double gam;
-                        if (flow_gamma(P, L, r_e, 1.0, 0.0, yn.pr, gam)) g_disk = gam;
+                        double igam;
+                        if (flow_igamma(P, L, r_e, 1.0, 0.0, yn.pr, igam)) g_disk = 1.0 / igam;
                     } else {
                         mode = radial_event(P, yn); loc_it = 0;
                     }
@@ -167,29 +217,38 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     mode = M_NORMAL;
                 }
             }
-            if (retake) continue;
+            commit = !retake;
+        }
 
-            // -------------------------------------------------------------- commit the step
-            if (KIND == 2) {
-                RtPoint pt; rt_point(P, L, yn.r, sn, cn, yn.pr, pt);
-                bool all_opaque = true;
-                if (SPEC) {
-                    for (int k = 0; k < nf; ++k) {
-                        double a1, e1; rt_coefficients(P, pt, P.nu[k], a1, e1);
+        // ------------------------------------------------------------------ radiative transfer over the step taken
+        if (KIND == 2 && (commit || fresh)) {
+            RtPoint pt; rt_point(P, L, yn.r, sn, cn, yn.pr, pt);
+            bool all_opaque = true;
+            if (SPEC) {
+                for (int k = 0; k < nf; ++k) {
+                    double a1, e1; rt_coefficients(P, pt, P.nu[k], P.ln_nu[k], a1, e1);
+                    if (commit) {
                         double tk = ACC(0, k), Tk = ACC(1, k), Ik = ACC(2, k);
                         rt_update(ACC(3, k), a1, ACC(4, k), e1, h_try, P.tau_max, tk, Tk, Ik);
-                        ACC(0, k) = tk; ACC(1, k) = Tk; ACC(2, k) = Ik; ACC(3, k) = a1; ACC(4, k) = e1;
+                        ACC(0, k) = tk; ACC(1, k) = Tk; ACC(2, k) = Ik;
                         if (!(tk > P.tau_max)) all_opaque = false;
                     }
-                } else {
-                    double a1, e1; rt_coefficients(P, pt, P.nu[0], a1, e1);
+                    ACC(3, k) = a1; ACC(4, k) = e1;
+                }
+            } else {
+                double a1, e1; rt_coefficients(P, pt, P.nu[0], P.ln_nu[0], a1, e1);
+                if (commit) {
                     rt_update(a0, a1, e0, e1, h_try, P.tau_max, tau, Tr, Inu);
-                    a0 = a1; e0 = e1;
                     all_opaque = (tau > P.tau_max);
                 }
-                if (flag < 0 && all_opaque) flag = F_OPAQUE;
+                a0 = a1; e0 = e1;
             }
-            y = yn; k1 = kn; cos_y = cn; h_try = h_next;
+            if (commit && flag < 0 && all_opaque) flag = F_OPAQUE;
+        }
+        if (commit || fresh) {                                         // (fresh: yn = y)
+            y = yn; cos_y = cn; kph0 = kn.ph;
+            K.set(0, 0, kn.r); K.set(1, 0, kn.th); K.set(2, 0, kn.pr); K.set(3, 0, kn.pth);
+            if (commit) h_try = h_next; else mode = M_NORMAL;
         }
 
         // ------------------------------------------------------------------ ray ended: outputs, release the lane

@@ -17,7 +17,7 @@ struct Params {
     double sin_obs, cos_obs, sin_pobs, cos_pobs, phi_obs;
     double x_min, x_span, y_min, y_span;        // x = x_min + (i + 1/2) x_span / nx
     double pix_area;
-    double rtol, h0, r_h, r_cap, r_esc;
+    double rtol, inv_rtol, h0, r_h, r_cap, r_esc;
     int32_t nx, ny, tiles_x, max_attempts;
     long long n_queue;                          // tiles_x * tiles_y * 32 queue slots
     // ---- flow (BASELINE.json:configs[2] "plunging inside")
@@ -26,17 +26,20 @@ struct Params {
     double r_in, r_out, emis_index, g_power, g_lo, g_hi, bins_per_g;
     int32_t nbins, kind;
     // ---- RIAF thermal synchrotron (eqs. (37)-(39); BASELINE.json:configs[2])
-    double n0, n_index, T0, T_index, inv_2h2;   // exp(-cos^2 θ * inv_2h2)
-    double B2_coef;                             // B^2 = B2_coef n_e / r
-    double theta_per_K;                         // Θ_e = theta_per_K T_e
-    double nuc_coef;                            // ν_c = nuc_coef B Θ_e^2, eq. (39)
-    double j_coef;                              // j = j_coef ν0 n_e M(x_M) / K_2(1/Θ_e), eq. (37) per steradian
-    double planck_coef;                         // 2h/c^2
-    double h_over_k;                            // h/k_B
+    // (log-space assembly of the emissivity: emission.cuh header)
+    double n_index, T_index, inv_2h2;           // n_e ∝ (r/r_h)^n_index exp(-cos²θ inv_2h2), T_e ∝ (r/r_h)^T_index
+    double ln_rh;                               // ln r_h
+    double ln_n0;                               // ln n0
+    double ln_Theta0;                           // ln(k_B T0 / m_e c²)
+    double ln_nuc0;                             // ln(3e/(4π m_e c)) + ½ ln(8π m_p c²/(6β)): ν_c = e^ln_nuc0 (n_e/r)^½ Θ_e², eq. (39)
+    double ln_j0;                               // ln(4.0505 j_scale e²/(√3 c)): eq. (37) per steradian × the 4.0505 of eq. (38)
+    double h_over_mc2;                          // h/(m_e c²): hν0/kT_e = h_over_mc2 ν0 /Θ_e
+    double inv_planck;                          // c²/(2h)
     double r_rt_out, tau_max, rg_cm;
     double sed_coef;                            // 4π r_g^2 Δx Δy
     int32_t nf, pad;
     double nu[MAX_FREQ];
+    double ln_nu[MAX_FREQ];
     double nu3[MAX_FREQ];                       // ν^3 (observed), image = ν^3 × invariant intensity
 };
 
