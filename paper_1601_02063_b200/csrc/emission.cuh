@@ -63,11 +63,14 @@ __device__ __forceinline__ bool flow_igamma(const Params& P, const double L, con
 }
 
 #define ODY_X(i, v) v,
+__constant__ double kK2A[ODY_K2_NS] = { ODY_K2_A(ODY_X) };
+__constant__ double kK2B[ODY_K2_NS] = { ODY_K2_B(ODY_X) };
+__constant__ double kK2P[ODY_K2_NC + 1] = { ODY_K2_P(ODY_X) };
+#undef ODY_X
 // 1/K_2(x) = kfac · exp(kexp) for 0 < x; lx = ln x.
 __device__ __forceinline__ void bessel_k2_inv(const double x, const double lx, double& kfac, double& kexp) {
     if (x <= 2.0) {
-        const double ca[ODY_K2_NS] = { ODY_K2_A(ODY_X) };
-        const double cb[ODY_K2_NS] = { ODY_K2_B(ODY_X) };
+        const double* const ca = kK2A; const double* const cb = kK2B;
         const double t = 0.25 * x * x;
         const double lg = lx - 0.69314718055994530942;               // ln(x/2)
         double A = 0.0, B = 0.0;
@@ -78,7 +81,7 @@ __device__ __forceinline__ void bessel_k2_inv(const double x, const double lx, d
         kfac = d_rcp(S);
         kexp = 2.0 * lx;
     } else {
-        const double cp[ODY_K2_NC + 1] = { ODY_K2_P(ODY_X) };
+        const double* const cp = kK2P;
         const double z = fma(4.0, d_rcp(x), -1.0);
         double F = 0.0;
 #pragma unroll
@@ -88,7 +91,6 @@ __device__ __forceinline__ void bessel_k2_inv(const double x, const double lx, d
         kexp = x + fma(0.5, lx, -0.22579135264472743236);            // ½ ln(2/π) = −0.2257913526…
     }
 }
-#undef ODY_X
 
 // What all frequencies share at one point of the ray.
 struct RtPoint {

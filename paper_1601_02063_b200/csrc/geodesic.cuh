@@ -101,6 +101,23 @@ __host__ __device__ constexpr double rk_b4(int j) {
     }
 }
 
+// The same coefficients as __constant__ tables: the kernels read kRkA[TAB][i][j] etc. (compile-time
+// indices; the constexpr functions above only prune the zero entries), so that the compiler loads them
+// with LDCU.128 into uniform registers once, outside the stage loop, instead of building every
+// 64-bit literal from two 32-bit immediates at each use.
+#define ODY_ROW(T, i) { rk_a<T>(i, 0), rk_a<T>(i, 1), rk_a<T>(i, 2), rk_a<T>(i, 3), rk_a<T>(i, 4), 0.0 }
+#define ODY_TABA(T) { ODY_ROW(T, 0), ODY_ROW(T, 1), ODY_ROW(T, 2), ODY_ROW(T, 3), ODY_ROW(T, 4), ODY_ROW(T, 5) }
+#define ODY_B5(T) { rk_b5<T>(0), rk_b5<T>(1), rk_b5<T>(2), rk_b5<T>(3), rk_b5<T>(4), rk_b5<T>(5) }
+#define ODY_BE(T) { rk_b5<T>(0) - rk_b4<T>(0), rk_b5<T>(1) - rk_b4<T>(1), rk_b5<T>(2) - rk_b4<T>(2), \
+                    rk_b5<T>(3) - rk_b4<T>(3), rk_b5<T>(4) - rk_b4<T>(4), rk_b5<T>(5) - rk_b4<T>(5) }
+__constant__ double kRkA[2][6][6] = { ODY_TABA(0), ODY_TABA(1) };
+__constant__ double kRkB5[2][6] = { ODY_B5(0), ODY_B5(1) };
+__constant__ double kRkBE[2][6] = { ODY_BE(0), ODY_BE(1) };
+#undef ODY_ROW
+#undef ODY_TABA
+#undef ODY_B5
+#undef ODY_BE
+
 // The four dynamic components' slopes of the six stages (φ does not enter the right-hand side, so its
 // stage values are never formed; only its two weighted sums are accumulated by the kernel).
 // Two storage policies with the same interface:
@@ -127,8 +144,8 @@ __device__ __forceinline__ void stage_point(const KS& K, const State& y, const d
     double sr = 0.0, st = 0.0, sp = 0.0, sq = 0.0;
 #pragma unroll
     for (int j = 0; j < I; ++j) {
-        const double aij = rk_a<TAB>(I, j);
-        if (aij != 0.0) {
+        if (rk_a<TAB>(I, j) != 0.0) {
+            const double aij = kRkA[TAB][I][j];
             sr = fma(aij, K.get(0, j), sr); st = fma(aij, K.get(1, j), st);
             sp = fma(aij, K.get(2, j), sp); sq = fma(aij, K.get(3, j), sq);
         }
@@ -144,13 +161,14 @@ __device__ __forceinline__ void rk_combine(const KS& K, const State& y, const do
     double s5[4] = {0.0, 0.0, 0.0, 0.0}, se[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-        const double b5 = rk_b5<TAB>(j), be = rk_b5<TAB>(j) - rk_b4<TAB>(j);
-        if (b5 != 0.0 || be != 0.0) {
+        const bool has5 = rk_b5<TAB>(j) != 0.0, hase = (rk_b5<TAB>(j) - rk_b4<TAB>(j)) != 0.0;
+        if (has5 || hase) {
+            const double b5 = kRkB5[TAB][j], be = kRkBE[TAB][j];
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 const double k = K.get(c, j);
-                if (b5 != 0.0) s5[c] = fma(b5, k, s5[c]);
-                if (be != 0.0) se[c] = fma(be, k, se[c]);
+                if (has5) s5[c] = fma(b5, k, s5[c]);
+                if (hase) se[c] = fma(be, k, se[c]);
             }
         }
     }

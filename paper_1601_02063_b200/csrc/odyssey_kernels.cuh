@@ -49,9 +49,8 @@ __device__ __forceinline__ int radial_event(const Params& P, const State& yn) {
 template <int TAB, int I, class KS>
 __device__ __forceinline__ void store_stage(KS& K, const Slope& k, double& ph5, double& phe) {
     K.set(0, I, k.r); K.set(1, I, k.th); K.set(2, I, k.pr); K.set(3, I, k.pth);
-    constexpr double b5 = rk_b5<TAB>(I), be = rk_b5<TAB>(I) - rk_b4<TAB>(I);
-    if (b5 != 0.0) ph5 = fma(b5, k.ph, ph5);
-    if (be != 0.0) phe = fma(be, k.ph, phe);
+    if (rk_b5<TAB>(I) != 0.0) ph5 = fma(kRkB5[TAB][I], k.ph, ph5);
+    if (rk_b5<TAB>(I) - rk_b4<TAB>(I) != 0.0) phe = fma(kRkBE[TAB][I], k.ph, phe);
 }
 
 template <int KIND, int TAB, bool SPEC, int NT, int MINB>
@@ -129,8 +128,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         bool run = active && !fresh;                                   // takes part in stages 2..6
         if (run && mode == M_NORMAL && n_att >= P.max_attempts) { flag = F_MAXSTEP; run = false; }
         bool done = false;                                             // end state evaluated: go on to events / commit
-        double ph5 = rk_b5<TAB>(0) * kph0;
-        double phe = (rk_b5<TAB>(0) - rk_b4<TAB>(0)) * kph0;
+        double ph5 = kRkB5[TAB][0] * kph0;
+        double phe = kRkBE[TAB][0] * kph0;
         State yn; Slope kn; double sn, cn;                             // defined in slot 6, read only when `done`
 
 #pragma unroll 1
