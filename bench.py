@@ -49,14 +49,24 @@ def parse_args():
     p.add_argument("--impl", default="b200", choices=["b200", "reference"])
     p.add_argument("--n", type=int, default=4096, help="image side (C4 sweep: 1024, 2048, 4096)")
     p.add_argument("--a", type=float, default=0.998, help="spin (C4 sweep: 0, 0.5, 0.9, 0.998)")
+    p.add_argument("--model", default="riaf", choices=["riaf", "none"],
+                   help="riaf: the fused geodesic + GRRT kernel (the headline); none: geodesics only (the paper's Table 1 workload)")
     p.add_argument("--cpu-sample", type=int, default=320, help="side of the strided sub-grid the oracle is timed on")
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     return p.parse_args()
 
 
-def workload_name(n, a):
-    return f"C4: Kerr a={a:g}, i=85deg, {n}x{n} over +/-15M, r_obs=1000M, RIAF 230 GHz, RKF45 rtol 1e-8"
+def workload_name(n, a, model="riaf"):
+    what = "RIAF 230 GHz" if model == "riaf" else "geodesics only"
+    return f"C4: Kerr a={a:g}, i=85deg, {n}x{n} over +/-15M, r_obs=1000M, {what}, RKF45 rtol 1e-8"
+
+
+def workload(args):
+    w = W.C4(n=args.n, a=args.a)
+    if args.model == "none":
+        w = dict(w, model=W.model_none(), nu=[0.0])
+    return w
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -145,7 +155,7 @@ def run_reference(args):
         return 0
     from oracle import build as oracle_build
     oracle_build.build()
-    w = W.C4(n=args.n, a=args.a)
+    w = workload(args)
     n_sub = args.cpu_sample
     for _ in range(min(args.warmup, 1)):
         time_oracle_sample(w, 64)
@@ -159,7 +169,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": tot_t / args.steps * 1e3,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": workload_name(args.n, args.a), "sample": sample},
+            "data": "synthetic", "config": {"workload": workload_name(args.n, args.a, args.model), "sample": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -193,7 +203,7 @@ def run_b200(args):
     ody.load_library()
     # Rays are independent: ranks share nothing; each rank renders one whole image per
     # step (weak scaling, no data-path collective — DESIGN.md §9).
-    w = W.C4(n=args.n, a=args.a)
+    w = workload(args)
     sc, mo, nu = w["scene"], w["model"], w["nu"][0]
     out = ody.render_image(sc, mo, nu)
     torch.cuda.synchronize()
@@ -266,15 +276,16 @@ def run_b200(args):
 
     ms_per_step = total_ms_max / args.steps
     value = ms_per_step * 1e6 / attempts_all                          # ns per photon per attempted RK step
-    flop_step = FLOP_PER_ATTEMPT_GEODESIC * attempts + FLOP_PER_RT_UPDATE * accepts     # per launch (this rank)
+    flop_rt = FLOP_PER_RT_UPDATE if args.model == "riaf" else 0.0
+    flop_step = FLOP_PER_ATTEMPT_GEODESIC * attempts + flop_rt * accepts                # per launch (this rank)
     kernel_ms = sum(step_ms) / len(step_ms)
     achieved = flop_step / (kernel_ms * 1e-3) / 1e12
-    info = ody.kernel_info(2, False, sc["tableau"])
+    info = ody.kernel_info(mo["kind"], False, sc["tableau"])
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(args.n, args.a), "photons_per_step": int(rays_all),
+        "config": {"workload": workload_name(args.n, args.a, args.model), "photons_per_step": int(rays_all),
                    "attempted_rk_steps_per_step": int(attempts_all), "accepted_rk_steps_per_step": int(accepts_all),
                    "attempts_per_photon": attempts_all / rays_all,
                    "l2": "no input arrays (rays are generated from the pixel index); the %d MB of per-step "
@@ -284,8 +295,8 @@ def run_b200(args):
         "ns_per_photon_per_accepted_step": ms_per_step * 1e6 / accepts_all,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                      "frac": achieved / peak_tflops, "traffic": None,
-                     "kernel": "odyssey_kernel<KIND=2,TAB=0,SPEC=false>", "kernel_ms": kernel_ms,
-                     "flop_per_attempt": FLOP_PER_ATTEMPT_GEODESIC, "flop_per_rt_update": FLOP_PER_RT_UPDATE,
+                     "kernel": "odyssey_kernel<KIND=%d,TAB=0,SPEC=false>" % mo["kind"], "kernel_ms": kernel_ms,
+                     "flop_per_attempt": FLOP_PER_ATTEMPT_GEODESIC, "flop_per_rt_update": flop_rt,
                      "peak_source": "odyssey_fp64_peak_probe (DFMA microbenchmark) in this run, best of 5"},
         "kernel_info": info,
         "gpu_launches": int(launches_all),

@@ -18,7 +18,7 @@ from . import build as _build
 EXPORTED_SYMBOLS = (
     "odyssey_trace_geodesics", "odyssey_render_image", "odyssey_render_spectrum",
     "odyssey_trace_geodesics_host", "odyssey_render_image_host", "odyssey_render_spectrum_host",
-    "odyssey_fp64_peak_probe", "odyssey_kernel_info", "odyssey_launch_count",
+    "odyssey_fp64_peak_probe", "odyssey_kernel_info", "odyssey_eval_math", "odyssey_launch_count",
     "odyssey_last_error", "odyssey_shutdown",
 )
 
@@ -86,7 +86,8 @@ def load_library():
     L.odyssey_launch_count.restype = C.c_longlong
     L.odyssey_last_error.restype = C.c_char_p
     L.odyssey_shutdown.restype = None
-    for name in EXPORTED_SYMBOLS[:8]:
+    L.odyssey_eval_math.argtypes = [C.c_int, C.c_int, dp, dp, dp, vp]
+    for name in EXPORTED_SYMBOLS[:9]:
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -220,6 +221,15 @@ def fp64_peak_probe(iters, sink):
     flop = C.c_double(0.0)
     _check(load_library().odyssey_fp64_peak_probe(C.c_int(int(iters)), _ptr(sink), C.byref(flop), _stream(torch)))
     return flop.value
+
+
+def eval_math(op, x):
+    """odyssey_eval_math on a CUDA float64 tensor; returns (y, y2)."""
+    torch = _torch()
+    x = x.contiguous()
+    y, y2 = torch.empty_like(x), torch.empty_like(x)
+    _check(load_library().odyssey_eval_math(C.c_int(int(op)), C.c_int(x.numel()), _ptr(x), _ptr(y), _ptr(y2), _stream(torch)))
+    return y, y2
 
 
 def kernel_info(kind, spectrum=False, tableau=0):

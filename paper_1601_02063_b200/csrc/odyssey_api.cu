@@ -324,6 +324,18 @@ int odyssey_fp64_peak_probe(int iters, double* sink, double* flop_host, void* cu
     return ODYSSEY_OK;
 }
 
+int odyssey_eval_math(int op, int n, const double* x, double* y, double* y2, void* cuda_stream) {
+    if (op < 0 || op > 7 || n < 0 || (n > 0 && (!x || !y)) || (op == 3 && !y2))
+        return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "eval_math: op in [0,7], n >= 0, x and y non-NULL (y2 too for op 3)");
+    if (n == 0) return ODYSSEY_OK;
+    DevState* D = nullptr;
+    TRY(device_state(&D, nullptr));
+    eval_math_kernel<<<(n + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(op, n, x, y, y2);
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+    return ODYSSEY_OK;
+}
+
 int odyssey_kernel_info(int kind, int spectrum, int tableau, int32_t* regs, int32_t* local_bytes,
                         int32_t* threads_per_block, int32_t* blocks_per_sm, int32_t* n_sm) {
     if (kind < 0 || kind > 2 || (tableau != 0 && tableau != 1)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown kind/tableau");

@@ -300,6 +300,26 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     }
 }
 
+// Diagnostic kernel behind odyssey_eval_math: the device elementary functions, elementwise.
+__global__ void eval_math_kernel(int op, int n, const double* __restrict__ x, double* __restrict__ y, double* __restrict__ y2) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double v = x[i];
+    double r = 0.0, r2 = 0.0;
+    switch (op) {
+        case 0: r = d_rcp(v); break;
+        case 1: r = d_rsqrt(v); break;
+        case 2: r = d_sqrt(v); break;
+        case 3: d_sincos(v, r, r2); break;
+        case 4: r = d_exp(v); break;
+        case 5: r = d_expm1(v); break;
+        case 6: r = d_log(v); break;
+        default: { double kf, ke; bessel_k2_inv(v, d_log(v), kf, ke); r = d_rcp(kf) * d_exp(-ke); }
+    }
+    y[i] = r;
+    if (y2) y2[i] = r2;
+}
+
 // FP64 peak probe: 16 independent DFMA chains per thread (BASELINE.json:north_star).
 __global__ void __launch_bounds__(256) dfma_probe_kernel(int iters, double* sink) {
     double v[16];
