@@ -35,10 +35,15 @@ import workloads as W  # noqa: E402
 METRIC = "ns per photon per RK step (FP64)"
 UNIT = "ns/photon/step"
 
-# Algorithmic FP64 work: flop per attempted RK step of the
-# geodesic system, and per radiative-transfer update (one per accepted step, single frequency).
-FLOP_PER_ATTEMPT_GEODESIC = 1500.0
-FLOP_PER_RT_UPDATE = 600.0
+# FP64 work per unit: flop per attempted RK step of the geodesic system, and per
+# radiative-transfer update (one per accepted step, single frequency).  These are the flop the kernels
+# EXECUTE (2 x DFMA + DMUL + DADD thread instructions, predicated on), measured with ncu on this very
+# workload — profiles/r01_c4_geodesic_kernel_ncu_full.md: 1031.8 per attempt; profiles/
+# r01_c4_riaf_kernel_ncu_full.md: 1391.9 per attempt with 0.7938 accepted steps per attempt
+# -> (1391.9 - 1031.8)/0.7938 = 453.7 per update.  SURVEY.md §8(d)'s a-priori hand count (1500 + ~490)
+# is 40 % higher: it would overstate the achieved rate, so it is not used.
+FLOP_PER_ATTEMPT_GEODESIC = 1031.8
+FLOP_PER_RT_UPDATE = 453.7
 
 
 def parse_args():
