@@ -130,11 +130,14 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         bool done = false;                                             // end state evaluated: go on to events / commit
         double ph5 = kRkB5[TAB][0] * kph0;
         double phe = kRkBE[TAB][0] * kph0;
-        State yn; Slope kn; double sn, cn;                             // defined in slot 6, read only when `done`
+        // The stage argument (ir, ith, ipr, ipth), the slope k and sinθ, cosθ are declared OUTSIDE the stage
+        // loop: after its last trip they hold the end state and f(end state), so no second set of
+        // loop-carried registers (and no copies at the loop head) is needed for them.
+        double ir, ith, ipr, ipth, yn_ph = y.ph;
+        Slope k; double sn, cn;
 
 #pragma unroll 1
         for (int s = 1; s <= 6; ++s) {
-            double ir = y.r, ith = y.th, ipr = y.pr, ipth = y.pth;
             bool ev = run;
             switch (s) {
                 case 1: stage_point<TAB, 1>(K, y, h_try, ir, ith, ipr, ipth); break;
@@ -144,7 +147,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                 case 5: stage_point<TAB, 5>(K, y, h_try, ir, ith, ipr, ipth); break;
                 default: {
                     if (run) {
-                        State ye;
+                        State yn, ye;
                         rk_combine<TAB>(K, y, h_try, ph5, phe, yn, ye);
                         ++n_att;
                         if (mode == M_NORMAL) {
@@ -159,26 +162,28 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                         } else {
                             ++loc_it;
                         }
+                        ir = yn.r; ith = yn.th; ipr = yn.pr; ipth = yn.pth; yn_ph = yn.ph;
+                    } else {                                           // a fresh lane evaluates f(y0) here
+                        ir = y.r; ith = y.th; ipr = y.pr; ipth = y.pth;
                     }
-                    if (!run) yn = y;                                  // a fresh lane evaluates f(y0) here
                     ev = ev || fresh;
                     done = ev;
-                    ir = yn.r; ith = yn.th; ipr = yn.pr; ipth = yn.pth;
                 }
             }
             if (ev) {
-                Slope k; double s_, c_;
-                geodesic_rhs(a, a2, L, ir, ith, ipr, ipth, k, s_, c_);
+                geodesic_rhs(a, a2, L, ir, ith, ipr, ipth, k, sn, cn);
                 switch (s) {
                     case 1: store_stage<TAB, 1>(K, k, ph5, phe); break;
                     case 2: store_stage<TAB, 2>(K, k, ph5, phe); break;
                     case 3: store_stage<TAB, 3>(K, k, ph5, phe); break;
                     case 4: store_stage<TAB, 4>(K, k, ph5, phe); break;
                     case 5: store_stage<TAB, 5>(K, k, ph5, phe); break;
-                    default: kn = k; sn = s_; cn = c_;
+                    default: break;
                 }
             }
         }
+        State yn; yn.r = ir; yn.th = ith; yn.ph = yn_ph; yn.pr = ipr; yn.pth = ipth;   // valid when `done`
+        const Slope& kn = k;
 
         // ------------------------------------------------------------------ events on the evaluated end state
         bool commit = false;
