@@ -67,6 +67,29 @@ ODY_HD uint64_t d_to_bits(double d) {
     uint64_t u; __builtin_memcpy(&u, &d, 8); return u;
 #endif
 }
+ODY_HD int32_t d_lo_word(double d) {
+#if defined(__CUDA_ARCH__)
+    return __double2loint(d);
+#else
+    return (int32_t)(uint32_t)d_to_bits(d);
+#endif
+}
+// x with its sign flipped when bit 31 of `mask_hi` is set (one LOP3 on the high word)
+ODY_HD double d_xor_sign(double x, uint32_t mask_hi) {
+#if defined(__CUDA_ARCH__)
+    return __hiloint2double(__double2hiint(x) ^ (int)(mask_hi & 0x80000000u), __double2loint(x));
+#else
+    return d_from_bits(d_to_bits(x) ^ ((uint64_t)(mask_hi & 0x80000000u) << 32));
+#endif
+}
+// 2^k for -1022 <= k <= 1023
+ODY_HD double d_pow2i(int32_t k) {
+#if defined(__CUDA_ARCH__)
+    return __hiloint2double((k + 1023) << 20, 0);
+#else
+    return d_from_bits((uint64_t)(uint32_t)(k + 1023) << 52);
+#endif
+}
 ODY_HD double d_fma(double a, double b, double c) {
 #if defined(__CUDA_ARCH__)
     return fma(a, b, c);
@@ -122,7 +145,7 @@ ODY_HD void d_sincos(double x, double& sn, double& cs) {
     const double* const S = kSinS; const double* const C = kCosC;
     const double MAGIC = kDm[0];
     const double t = d_fma(x, kDm[1], MAGIC);                      // x * 2/pi
-    const int32_t q = (int32_t)(uint32_t)d_to_bits(t);             // low word = nearest integer
+    const int32_t q = d_lo_word(t);                                // low word = nearest integer
     const double k = t - MAGIC;
     double r = d_fma(-k, kDm[2], x);                               // pi/2 high part
     r = d_fma(-k, kDm[3], r);                                      // pi/2 low part
@@ -135,21 +158,20 @@ ODY_HD void d_sincos(double x, double& sn, double& cs) {
     const double sr = d_fma(ps * z, r, r);                         // r + r^3 S(z)
     const double cr = d_fma(z * z, pc, d_fma(-0.5, z, 1.0));       // 1 - z/2 + z^2 C(z)
     const bool swap = q & 1;
-    double s0 = swap ? cr : sr, c0 = swap ? sr : cr;
-    if (q & 2) s0 = -s0;
-    if ((q + 1) & 2) c0 = -c0;
-    sn = s0; cs = c0;
+    const double s0 = swap ? cr : sr, c0 = swap ? sr : cr;
+    sn = d_xor_sign(s0, (uint32_t)q << 30);                        // negative in quadrants 2, 3
+    cs = d_xor_sign(c0, (uint32_t)(q + 1) << 30);                  // negative in quadrants 1, 2
 }
 
 // x = k ln2 + r with |r| <= ln2/2; returns r and 2^k (as a double), for |x| <= ~700.
 ODY_HD double d_exp_reduce(double x, double& two_k) {
     const double MAGIC = kDm[0];
     const double t = d_fma(x, kDm[4], MAGIC);
-    const int32_t k = (int32_t)(uint32_t)d_to_bits(t);
+    const int32_t k = d_lo_word(t);
     const double kf = t - MAGIC;
     double r = d_fma(-kf, kDm[5], x);
     r = d_fma(-kf, kDm[6], r);
-    two_k = d_from_bits((uint64_t)(uint32_t)(k + 1023) << 52);
+    two_k = d_pow2i(k);
     return r;
 }
 
@@ -163,22 +185,32 @@ ODY_HD double d_expq(double r) {                                   // (e^r - 1)/
     return p;
 }
 
-// e^x; arguments below -700 return 0, above 700 are clamped (callers never get there with finite results).
-ODY_HD double d_exp(double x) {
-    const double xc = x < -700.0 ? -700.0 : (x > 700.0 ? 700.0 : x);
+// e^x for |x| <= 700 (no range check: the caller knows the range).
+ODY_HD double d_exp_nc(double x) {
     double two_k;
-    const double r = d_exp_reduce(xc, two_k);
-    const double v = d_fma(r * d_expq(r), two_k, two_k);           // 2^k (1 + r q)
-    return x < -700.0 ? 0.0 : v;
+    const double r = d_exp_reduce(x, two_k);
+    return d_fma(r * d_expq(r), two_k, two_k);                     // 2^k (1 + r q)
 }
 
-// e^x - 1, accurate near 0; same argument range as d_exp.
-ODY_HD double d_expm1(double x) {
-    const double xc = x < -700.0 ? -700.0 : (x > 700.0 ? 700.0 : x);
+// e^x for x <= 700; arguments below -700 (and NaN) return 0.
+ODY_HD double d_exp_lo(double x) {
+    const bool ok = x >= -700.0;
+    const double v = d_exp_nc(ok ? x : -700.0);
+    return ok ? v : 0.0;
+}
+
+// e^x; arguments below -700 return 0, above 700 are clamped.
+ODY_HD double d_exp(double x) { return d_exp_lo(x > 700.0 ? 700.0 : x); }
+
+// e^x - 1, accurate near 0, for |x| <= 700.
+ODY_HD double d_expm1_nc(double x) {
     double two_k;
-    const double r = d_exp_reduce(xc, two_k);
+    const double r = d_exp_reduce(x, two_k);
     return d_fma(r * d_expq(r), two_k, two_k - 1.0);               // 2^k r q + (2^k - 1)
 }
+
+// e^x - 1 with the argument clamped to [-700, 700] (e^-700 - 1 = -1 exactly in FP64).
+ODY_HD double d_expm1(double x) { return d_expm1_nc(x < -700.0 ? -700.0 : (x > 700.0 ? 700.0 : x)); }
 
 // natural logarithm of a normal x > 0.
 ODY_HD double d_log(double x) {

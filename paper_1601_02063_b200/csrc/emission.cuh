@@ -112,8 +112,9 @@ __device__ __forceinline__ void rt_point(const Params& P, const double L, const 
     const double lrel = lr - P.ln_rh;                               // ln(r / r_h)
     const double ln_ne = fma(P.n_index, lrel, fma(-c * c, P.inv_2h2, P.ln_n0));
     const double ln_Th = fma(P.T_index, lrel, P.ln_Theta0);         // ln Θ_e
-    if (!(ln_Th > -6.5)) return;                                    // 1/Θ_e > 665: K_2 underflows, no emission
-    const double x = d_exp(-ln_Th);                                 // 1/Θ_e
+    if (!(ln_Th > -6.5 && ln_Th < 690.0)) return;                   // 1/Θ_e > 665: K_2 underflows, no emission
+    if (!(ln_ne > -1e300)) return;                                  // n0 = 0
+    const double x = d_exp_nc(-ln_Th);                              // 1/Θ_e
     double kfac, kexp;
     bessel_k2_inv(x, -ln_Th, kfac, kexp);
     const double ligam = d_log(igam);
@@ -131,16 +132,18 @@ __device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& 
                                                 double& acoef, double& ecoef) {
     acoef = 0.0; ecoef = 0.0;
     if (!q.on) return;
-    const double t = d_exp((ln_nu + q.lxm0) * (1.0 / 12.0));        // x_M^(1/12)
+    const double t = d_exp_nc((ln_nu + q.lxm0) * (1.0 / 12.0));     // x_M^(1/12); |argument| < 700 always
     const double u = d_rcp(t);
     const double t2 = t * t, u2 = u * u;
     const double u3 = u2 * u;
     const double poly = fma(u3, fma(0.5316, u3, 0.40), 1.0);        // eq. (38) bracket
     const double ex = d_exp(fma(-1.8899, t2 * t2, fma(-2.0, ln_nu, q.E)));
     const double eps = q.fac * u2 * poly * ex;                       // reading D, F
-    const double em1 = d_expm1(nu * q.ycoef);                        // e^{hν0/kT} − 1
+    const double ya = nu * q.ycoef;                                  // hν0/kT_e >= 0
+    const bool planck_ok = ya < 700.0;                               // beyond: B_ν underflows, α = 0 as in the formula
+    const double em1 = d_expm1_nc(planck_ok ? ya : 700.0);           // e^{hν0/kT} − 1
     ecoef = eps;
-    acoef = (eps > 0.0 && nu * q.ycoef < 700.0) ? eps * em1 * P.inv_planck : 0.0;   // Kirchhoff
+    acoef = (eps > 0.0 && planck_ok) ? eps * em1 * P.inv_planck : 0.0;   // Kirchhoff
 }
 
 // Trapezoid in λ for Δτ and the emission, exact attenuation across the step: φ(x) = (1 − e^−x)/x.
@@ -148,7 +151,7 @@ __device__ __forceinline__ void rt_update(const double a0, const double a1, cons
                                           const double dl, const double tau_max, double& tau, double& T, double& I) {
     if (tau > tau_max) return;
     const double dtau = 0.5 * (a0 + a1) * dl;
-    const double em = d_expm1(-dtau);                                // e^−Δτ − 1
+    const double em = d_expm1_nc(dtau < 700.0 ? -dtau : -700.0);     // e^−Δτ − 1 (Δτ >= 0)
     const double phi = (dtau > 1e-300) ? -em * d_rcp(dtau) : 1.0;
     I = fma(T * (0.5 * (e0 + e1) * dl), phi, I);
     T = fma(T, em, T);

@@ -184,14 +184,22 @@ __device__ __forceinline__ double error_norm(const State& y, const State& e, con
     const double q1 = fabs(e.th), q2 = fabs(e.ph);
     const double q3 = fabs(e.pr) * d_rcp(1.0 + fabs(y.pr));
     const double q4 = fabs(e.pth) * d_rcp(1.0 + fabs(y.pth));
-    const double m = fmax(fmax(fmax(q0, q1), fmax(q2, q3)), q4);   // fmax drops NaNs …
-    const double sum = q0 + q1 + q2 + q3 + q4;                     // … so detect them here (all q ≥ 0)
+    // plain compare-and-select maxima (fmax's NaN rules cost a dozen instructions each); NaNs are caught below
+    double m = q0 > q1 ? q0 : q1;
+    const double m2 = q2 > q3 ? q2 : q3;
+    m = m > m2 ? m : m2;
+    m = m > q4 ? m : q4;
+    const double sum = q0 + q1 + q2 + q3 + q4;                     // NaN anywhere -> NaN here (all q >= 0)
     return (sum != sum) ? sum : m * inv_rtol;
 }
 
-// x^(-1/5) for x in (0, 1]: single-precision seed, two Newton steps y ← y (6 − x y⁵)/5 in FP64.
+// x^(-1/5) for x in (0, 1]: MUFU.LG2 / MUFU.EX2 seed in single precision (relative error ~1e-6), two
+// Newton steps y <- y (6 - x y^5)/5 in FP64 (error -> 3e^2 per step).
 __device__ __forceinline__ double inv_fifth_root(const double x) {
-    double y = (double)exp2f(-0.2f * log2f((float)x));
+    float l, sd;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"((float)x));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(sd) : "f"(-0.2f * l));
+    double y = (double)sd;
 #pragma unroll
     for (int it = 0; it < 2; ++it) {
         const double y2 = y * y;
@@ -199,6 +207,18 @@ __device__ __forceinline__ double inv_fifth_root(const double x) {
         y = y * fma(-x, y5, 6.0) * 0.2;
     }
     return y;
+}
+
+// Step-size factors of the controller (reading G), with compare-and-select clamps.
+__device__ __forceinline__ double grow_factor(const double err) {          // accepted: min(5, 0.9 err^-0.2)
+    if (err < 1.889568e-4) return 5.0;
+    const double f = 0.9 * inv_fifth_root(err);
+    return f < 5.0 ? f : 5.0;
+}
+__device__ __forceinline__ double shrink_factor(const double err) {        // rejected: max(0.1, 0.9 err^-0.25)
+    if (!(err < 1e300)) return 0.1;                                        // infinite or NaN
+    const double f = 0.9 * d_rsqrt(d_sqrt(err));
+    return f > 0.1 ? f : 0.1;
 }
 
 // ------------------------------------------------------------------------------------------------

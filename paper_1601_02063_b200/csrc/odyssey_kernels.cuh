@@ -153,11 +153,11 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                         if (mode == M_NORMAL) {
                             const double err = error_norm(y, ye, P.inv_rtol);
                             if (!(err <= 1.0)) {                       // reject (also NaN): shrink, keep k1
-                                h_try *= isfinite(err) ? fmax(0.1, 0.9 * d_rsqrt(d_sqrt(err))) : 0.1;
+                                h_try *= shrink_factor(err);
                                 ev = false;
                             } else {
                                 ++n_acc;
-                                h_next = h_try * ((err < 1.889568e-4) ? 5.0 : fmin(5.0, 0.9 * inv_fifth_root(err)));
+                                h_next = h_try * grow_factor(err);
                             }
                         } else {
                             ++loc_it;
