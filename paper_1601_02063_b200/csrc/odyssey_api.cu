@@ -151,7 +151,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
 }
 
 // ---- kernel table ------------------------------------------------------------------------------
-constexpr int NT_MAIN = 128, MINB_MAIN = 4;     // 128 registers per thread at most
+constexpr int NT_MAIN = 128, MINB_MAIN = 5;     // 96 registers per thread at most
 constexpr int NT_SPEC = 160, MINB_SPEC = 1;     // 5 x 32 x 160 x 8 B = 200 KiB of accumulators
 
 typedef void (*KernelFn)(const Params, const Outputs);
@@ -167,7 +167,7 @@ KernelFn pick_kernel(int kind, bool spec, int tab) {
 
 size_t smem_bytes(int kind, bool spec, int nf, int nbins) {
     if (spec) return (size_t)(5 * nf * NT_SPEC + MAX_FREQ) * sizeof(double);
-    const size_t stages = (size_t)24 * NT_MAIN * sizeof(double);         // [4][6][NT] stage slopes
+    const size_t stages = (size_t)29 * NT_MAIN * sizeof(double);         // [4][6][NT] stage slopes + [5][NT] RT state
     if (kind == 1) return stages + (size_t)(nbins > 0 ? nbins : 1) * sizeof(double);
     return stages;
 }

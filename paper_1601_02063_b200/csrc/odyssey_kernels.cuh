@@ -60,9 +60,11 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     const int lane = threadIdx.x & 31;
     const int nf = SPEC ? P.nf : 1;
     // shared layout: SPEC: [5][nf][NT] accumulators then sed[MAX_FREQ];
-    //                otherwise: [4][6][NT] stage slopes, then (KIND 1) hist[nbins]
+    //                otherwise: [4][6][NT] stage slopes, [5][NT] single-frequency RT state, then (KIND 1) hist[nbins]
     double* const sm_acc = smem;
-    double* const sm_red = SPEC ? smem + 5 * nf * NT : smem + 24 * NT;
+    double* const sm_red = SPEC ? smem + 5 * nf * NT : smem + 29 * NT;
+    double* const sm_rt = smem + 24 * NT + threadIdx.x;            // (!SPEC) q: 0 tau, 1 T, 2 I, 3 a0, 4 e0
+#define RT1(q) sm_rt[(q) * NT]
     if (SPEC) { for (int k = threadIdx.x; k < MAX_FREQ; k += NT) sm_red[k] = 0.0; }
     if (KIND == 1) { for (int k = threadIdx.x; k < P.nbins; k += NT) sm_red[k] = 0.0; }
     if (SPEC || KIND == 1) __syncthreads();
@@ -76,7 +78,6 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     if constexpr (!SPEC) K.base = smem + threadIdx.x;
     double kph0 = 0.0;                                              // φ slope of the cached first stage
     double L = 0.0, h_try = 0.0, h_next = 0.0, cos_y = 0.0;
-    double tau = 0.0, Tr = 1.0, Inu = 0.0, a0 = 0.0, e0 = 0.0;      // single-frequency RT state
     double g_disk = 0.0, r_e = 0.0;
     y.r = y.th = y.ph = y.pr = y.pth = 0.0;
 #pragma unroll
@@ -109,7 +110,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                             if (SPEC) {
                                 for (int k = 0; k < nf; ++k) { ACC(0, k) = 0.0; ACC(1, k) = 1.0; ACC(2, k) = 0.0; ACC(3, k) = 0.0; ACC(4, k) = 0.0; }
                             } else {
-                                tau = 0.0; Tr = 1.0; Inu = 0.0; a0 = 0.0; e0 = 0.0;
+                                RT1(0) = 0.0; RT1(1) = 1.0; RT1(2) = 0.0; RT1(3) = 0.0; RT1(4) = 0.0;
                             }
                         }
                         active = true;
@@ -242,10 +243,12 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             } else {
                 double a1, e1; rt_coefficients(P, pt, P.nu[0], P.ln_nu[0], a1, e1);
                 if (commit) {
-                    rt_update(a0, a1, e0, e1, h_try, P.tau_max, tau, Tr, Inu);
+                    double tau = RT1(0), Tr = RT1(1), Inu = RT1(2);
+                    rt_update(RT1(3), a1, RT1(4), e1, h_try, P.tau_max, tau, Tr, Inu);
+                    RT1(0) = tau; RT1(1) = Tr; RT1(2) = Inu;
                     all_opaque = (tau > P.tau_max);
                 }
-                a0 = a1; e0 = e1;
+                RT1(3) = a1; RT1(4) = e1;
             }
             if (commit && flag < 0 && all_opaque) flag = F_OPAQUE;
         }
@@ -279,8 +282,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     atomicAdd(&sm_red[b], val * P.pix_area);
                 }
             } else if (!SPEC) {
-                if (O.image) O.image[pix] = P.nu3[0] * Inu;
-                if (O.aux0) O.aux0[pix] = tau;
+                if (O.image) O.image[pix] = P.nu3[0] * RT1(2);
+                if (O.aux0) O.aux0[pix] = RT1(0);
                 if (O.aux1) O.aux1[pix] = 0.0;
             } else {
                 const size_t npix = (size_t)P.nx * P.ny;
@@ -294,6 +297,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         }
     }
 #undef ACC
+#undef RT1
     // ---------------------------------------------------------------------- block-level reductions
     if (SPEC && O.nuLnu) {
         __syncthreads();
