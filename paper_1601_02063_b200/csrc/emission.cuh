@@ -103,7 +103,7 @@ struct RtPoint {
 
 __device__ __forceinline__ void rt_point(const Params& P, const double L, const double r, const double s, const double c,
                                          const double pr, RtPoint& q) {
-    q.on = false;
+    q.on = false; q.fac = 0.0; q.E = 0.0; q.lxm0 = 0.0; q.ycoef = 0.0;     // off: every coefficient evaluates to 0
     if (!(r > P.r_cap && r < P.r_rt_out)) return;
     double igam;
     if (!flow_igamma(P, L, r, s, c, pr, igam)) return;
@@ -130,8 +130,8 @@ __device__ __forceinline__ void rt_point(const Params& P, const double L, const 
 // Per-frequency coefficients.  ln_nu = ln ν_k.
 __device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& q, const double nu, const double ln_nu,
                                                 double& acoef, double& ecoef) {
-    acoef = 0.0; ecoef = 0.0;
-    if (!q.on) return;
+    // straight-line on purpose (no early return when the point is off: fac = 0 gives ε = a = 0), so that the
+    // spectrum kernel's unrolled frequency loop can interleave independent chains
     const double t = d_exp_nc((ln_nu + q.lxm0) * (1.0 / 12.0));     // x_M^(1/12); |argument| < 700 always
     const double u = d_rcp(t);
     const double t2 = t * t, u2 = u * u;
@@ -149,13 +149,15 @@ __device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& 
 // Trapezoid in λ for Δτ and the emission, exact attenuation across the step: φ(x) = (1 − e^−x)/x.
 __device__ __forceinline__ void rt_update(const double a0, const double a1, const double e0, const double e1,
                                           const double dl, const double tau_max, double& tau, double& T, double& I) {
-    if (tau > tau_max) return;
+    const bool live = !(tau > tau_max);                              // a frozen frequency keeps its values (selects, no branch)
     const double dtau = 0.5 * (a0 + a1) * dl;
     const double em = d_expm1_nc(dtau < 700.0 ? -dtau : -700.0);     // e^−Δτ − 1 (Δτ >= 0)
     const double phi = (dtau > 1e-300) ? -em * d_rcp(dtau) : 1.0;
-    I = fma(T * (0.5 * (e0 + e1) * dl), phi, I);
-    T = fma(T, em, T);
-    tau += dtau;
+    const double In = fma(T * (0.5 * (e0 + e1) * dl), phi, I);
+    const double Tn = fma(T, em, T);
+    I = live ? In : I;
+    T = live ? Tn : T;
+    tau = live ? tau + dtau : tau;
 }
 
 }  // namespace ody

@@ -120,16 +120,9 @@ __constant__ double kRkBE[2][6] = { ODY_BE(0), ODY_BE(1) };
 
 // The four dynamic components' slopes of the six stages (φ does not enter the right-hand side, so its
 // stage values are never formed; only its two weighted sums are accumulated by the kernel).
-// Two storage policies with the same interface:
-//   StagesReg  : 24 doubles in registers (spectrum kernel: one block per SM, registers to spare);
-//   StagesSmem : 24 doubles per thread in shared memory, [component][stage][thread] — consecutive lanes
-//                hit consecutive 8-byte words, so every access is conflict-free.  This takes 48
-//                registers off the main kernel, which is what lets it run 4 blocks of 128 threads per SM.
-struct StagesReg {
-    double v[4][6];
-    __device__ __forceinline__ double get(int c, int j) const { return v[c][j]; }
-    __device__ __forceinline__ void set(int c, int j, double x) { v[c][j] = x; }
-};
+// They live in shared memory, [component][stage][thread] — consecutive lanes hit consecutive 8-byte
+// words, so every access is conflict-free.  This takes 48 registers off the kernel, which is what lets
+// it run 5 blocks of 128 threads per SM at 96 registers without spills.
 template <int NT>
 struct StagesSmem {
     double* base;                                       // &smem[threadIdx.x]
@@ -233,28 +226,29 @@ __device__ __forceinline__ void init_ray(const Params& P, const double x, const 
     const double zp = P.r_obs * P.cos_obs + yimg * P.sin_obs;
     // eqs. (20)-(22)
     const double w = xp * xp + yp * yp + zp * zp - a2;
-    const double r = sqrt(0.5 * (w + sqrt(w * w + 4.0 * a2 * zp * zp)));
-    const double th = acos(zp / r);
+    const double r = d_sqrt(0.5 * (w + d_sqrt(w * w + 4.0 * a2 * zp * zp)));
+    const double th = acos(zp * d_rcp(r));
     const double ph = atan2(yp, xp);
     // eqs. (24)-(26)
-    const double R = sqrt(r * r + a2);
+    const double R = d_sqrt(r * r + a2);
     double sP, cP, s, c;
-    sincos(ph - P.phi_obs, &sP, &cP);
-    sincos(th, &s, &c);
+    d_sincos(ph - P.phi_obs, sP, cP);
+    d_sincos(th, s, c);
     const double Sigma = r * r + a2 * c * c;
     const double Delta = r * r - 2.0 * r + a2;
-    const double rdot = -(r * R * s * P.sin_obs * cP + R * R * c * P.cos_obs) / Sigma;
-    const double thdot = (r * s * P.cos_obs - R * c * P.sin_obs * cP) / Sigma;
-    const double phdot = P.sin_obs * sP / (R * s);
+    const double iSig = d_rcp(Sigma), iDel = d_rcp(Delta), iS2r = d_rcp(Sigma - 2.0 * r);
+    const double rdot = -(r * R * s * P.sin_obs * cP + R * R * c * P.cos_obs) * iSig;
+    const double thdot = (r * s * P.cos_obs - R * c * P.sin_obs * cP) * iSig;
+    const double phdot = P.sin_obs * sP * d_rcp(R * s);
     // eq. (7), μ = 0; E = −sqrt(E²) (reading B); eq. (8); eqs. (4), (5)
-    const double E2 = ((Sigma - 2.0 * r) / (Sigma * Delta)) * (Sigma * rdot * rdot + Sigma * Delta * thdot * thdot)
+    const double E2 = ((Sigma - 2.0 * r) * iSig * iDel) * (Sigma * rdot * rdot + Sigma * Delta * thdot * thdot)
                     + Delta * phdot * phdot * s * s;
-    const double En = sqrt(E2);                                    // |E|
-    const double Lraw = (Sigma * Delta * phdot + 2.0 * a * r * En) * s * s / (Sigma - 2.0 * r);
-    const double inv = 1.0 / En;                                   // normalise to |E| = 1 (reading C)
+    const double inv = d_rsqrt(E2);                                // 1/|E|: normalise to |E| = 1 (reading C)
+    const double En = E2 * inv;                                    // |E|
+    const double Lraw = (Sigma * Delta * phdot + 2.0 * a * r * En) * s * s * iS2r;
     L = Lraw * inv;
     y.r = r; y.th = th; y.ph = ph;
-    y.pr = Sigma * rdot / Delta * inv;
+    y.pr = Sigma * rdot * iDel * inv;
     y.pth = Sigma * thdot * inv;
 }
 

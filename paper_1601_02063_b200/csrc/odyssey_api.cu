@@ -152,7 +152,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
 
 // ---- kernel table ------------------------------------------------------------------------------
 constexpr int NT_MAIN = 128, MINB_MAIN = 5;     // 96 registers per thread at most
-constexpr int NT_SPEC = 160, MINB_SPEC = 1;     // 5 x 32 x 160 x 8 B = 200 KiB of accumulators
+constexpr int NT_SPEC = 128, MINB_SPEC = 3;     // 168 registers (the unrolled frequency loop wants them); per-frequency accumulators in a global scratch buffer
 
 typedef void (*KernelFn)(const Params, const Outputs);
 
@@ -166,7 +166,7 @@ KernelFn pick_kernel(int kind, bool spec, int tab) {
 }
 
 size_t smem_bytes(int kind, bool spec, int nf, int nbins) {
-    if (spec) return (size_t)(5 * nf * NT_SPEC + MAX_FREQ) * sizeof(double);
+    if (spec) return (size_t)(29 * NT_SPEC + MAX_FREQ) * sizeof(double);
     const size_t stages = (size_t)29 * NT_MAIN * sizeof(double);         // [4][6][NT] stage slopes + [5][NT] RT state
     if (kind == 1) return stages + (size_t)(nbins > 0 ? nbins : 1) * sizeof(double);
     return stages;
@@ -193,8 +193,15 @@ int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
     CUDA_TRY(cudaMemsetAsync(O.queue, 0, sizeof(unsigned long long), st));
     if (O.hist && P.nbins > 0) CUDA_TRY(cudaMemsetAsync(O.hist, 0, sizeof(double) * P.nbins, st));
     if (O.nuLnu) CUDA_TRY(cudaMemsetAsync(O.nuLnu, 0, sizeof(double) * P.nf, st));
+    if (spec) {      // stream-ordered scratch for the per-frequency accumulators: [5][nf][blocks * nt] doubles
+        void* scratch = nullptr;
+        CUDA_TRY(cudaMallocAsync(&scratch, sizeof(double) * 5 * (size_t)P.nf * (size_t)blocks * nt, st));
+        O.spec_state = (double*)scratch;
+    }
     void* args[] = {(void*)&P, (void*)&O};
-    CUDA_TRY(cudaLaunchKernel((const void*)fn, dim3((unsigned)blocks), dim3(nt), args, sm, st));
+    cudaError_t le = cudaLaunchKernel((const void*)fn, dim3((unsigned)blocks), dim3(nt), args, sm, st);
+    if (spec) cudaFreeAsync(O.spec_state, st);
+    if (le != cudaSuccess) return fail(ODYSSEY_ERR_CUDA, "cudaLaunchKernel: %s", cudaGetErrorString(le));
     g_launches.fetch_add(1);
     return ODYSSEY_OK;
 }

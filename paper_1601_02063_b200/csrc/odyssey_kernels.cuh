@@ -23,8 +23,9 @@
 //   commit  : radiative-transfer update over the step actually taken (eqs. (30), (31)), state
 //             advance, outputs + release of the lane when the ray has ended.
 //
-// All per-ray state lives in registers; the spectrum variant keeps its 5 x nf per-frequency
-// accumulators in shared memory laid out [quantity][frequency][thread] (bank-conflict free).
+// Per-ray state: registers for what every stage touches (y, L, h, the φ sums); shared memory for the 24
+// stage slopes and the single-frequency transfer state; a global scratch buffer for the spectrum
+// variant's 5 x nf per-frequency accumulators.  No local memory.
 #pragma once
 #include <cuda_runtime.h>
 #include <type_traits>
@@ -59,23 +60,26 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31;
     const int nf = SPEC ? P.nf : 1;
-    // shared layout: SPEC: [5][nf][NT] accumulators then sed[MAX_FREQ];
-    //                otherwise: [4][6][NT] stage slopes, [5][NT] single-frequency RT state, then (KIND 1) hist[nbins]
-    double* const sm_acc = smem;
-    double* const sm_red = SPEC ? smem + 5 * nf * NT : smem + 29 * NT;
+    // shared layout: [4][6][NT] stage slopes, [5][NT] single-frequency RT state, then hist[nbins] (KIND 1)
+    // or sed[MAX_FREQ] (SPEC).  The spectrum variant's 5 x nf per-frequency accumulators live in a global
+    // scratch buffer laid out [quantity][frequency][grid thread] (every warp access is one contiguous
+    // 256-byte segment; 160 doubles per thread would cap the SM at 5 warps if they sat in shared memory).
+    double* const sm_red = smem + 29 * NT;
     double* const sm_rt = smem + 24 * NT + threadIdx.x;            // (!SPEC) q: 0 tau, 1 T, 2 I, 3 a0, 4 e0
+    const size_t spec_stride = (size_t)gridDim.x * NT;
+    double* const gl_acc = SPEC ? O.spec_state + (size_t)blockIdx.x * NT + threadIdx.x : nullptr;
 #define RT1(q) sm_rt[(q) * NT]
     if (SPEC) { for (int k = threadIdx.x; k < MAX_FREQ; k += NT) sm_red[k] = 0.0; }
     if (KIND == 1) { for (int k = threadIdx.x; k < P.nbins; k += NT) sm_red[k] = 0.0; }
     if (SPEC || KIND == 1) __syncthreads();
-#define ACC(q, k) sm_acc[((q) * nf + (k)) * NT + threadIdx.x]      // q: 0 tau, 1 T, 2 I, 3 a0, 4 e0
+#define ACC(q, k) gl_acc[((q) * nf + (k)) * spec_stride]            // q: 0 tau, 1 T, 2 I, 3 a0, 4 e0
 
     const double a = P.a, a2 = P.a2;
     bool active = false, exhausted = false, on_eq = false;
     int pix = 0, n_att = 0, n_acc = 0, mode = M_NORMAL, loc_it = 0;
     State y;
-    typename std::conditional<SPEC, StagesReg, StagesSmem<NT>>::type K;
-    if constexpr (!SPEC) K.base = smem + threadIdx.x;
+    StagesSmem<NT> K;
+    K.base = smem + threadIdx.x;
     double kph0 = 0.0;                                              // φ slope of the cached first stage
     double L = 0.0, h_try = 0.0, h_next = 0.0, cos_y = 0.0;
     double g_disk = 0.0, r_e = 0.0;
@@ -230,14 +234,16 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             RtPoint pt; rt_point(P, L, yn.r, sn, cn, yn.pr, pt);
             bool all_opaque = true;
             if (SPEC) {
+#pragma unroll 4
                 for (int k = 0; k < nf; ++k) {
+                    // loads first (their latency hides behind the coefficient evaluation), no branches: the
+                    // unrolled iterations are independent chains the scheduler can interleave
+                    double tk = ACC(0, k), Tk = ACC(1, k), Ik = ACC(2, k);
+                    const double a0k = ACC(3, k), e0k = ACC(4, k);
                     double a1, e1; rt_coefficients(P, pt, P.nu[k], P.ln_nu[k], a1, e1);
-                    if (commit) {
-                        double tk = ACC(0, k), Tk = ACC(1, k), Ik = ACC(2, k);
-                        rt_update(ACC(3, k), a1, ACC(4, k), e1, h_try, P.tau_max, tk, Tk, Ik);
-                        ACC(0, k) = tk; ACC(1, k) = Tk; ACC(2, k) = Ik;
-                        if (!(tk > P.tau_max)) all_opaque = false;
-                    }
+                    rt_update(a0k, a1, e0k, e1, commit ? h_try : 0.0, P.tau_max, tk, Tk, Ik);   // fresh lane: zero-length step
+                    ACC(0, k) = tk; ACC(1, k) = Tk; ACC(2, k) = Ik;
+                    if (!(tk > P.tau_max)) all_opaque = false;
                     ACC(3, k) = a1; ACC(4, k) = e1;
                 }
             } else {

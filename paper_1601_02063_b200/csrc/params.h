@@ -51,6 +51,7 @@ struct Outputs {
     double* image; double* aux0; double* aux1;   // single-frequency image modes
     double* hist;                                // kind 1
     double* images; double* nuLnu;               // spectrum mode
+    double* spec_state;                          // spectrum mode: library scratch, [5][nf][grid threads] accumulators
     unsigned long long* queue;                   // work-queue counter (zeroed before the launch)
 };
 
