@@ -183,6 +183,32 @@ def run_reference(args):
 
 
 # ---------------------------------------------------------------------------------------------------
+# rank reduction and headline arithmetic (plain functions: tests/test_bench_multirank.py runs them under
+# gloo with world_size 2 on CPU)
+# ---------------------------------------------------------------------------------------------------
+def reduce_over_ranks(dist, device, times, counts):
+    """times: per-rank durations -> MAX over ranks; counts: per-rank work -> SUM over ranks.
+    dist is torch.distributed (initialised) or None for a single process."""
+    import torch
+    t = torch.tensor(list(times), dtype=torch.float64, device=device)
+    n = torch.tensor(list(counts), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    return t.tolist(), n.tolist()
+
+
+def headline(total_ms_max, steps, attempts_all, accepts_all, world):
+    """Whole-job figures from the max-over-ranks time of `steps` steps and the per-step work summed over
+    ranks (every rank renders whole images of its own: weak scaling)."""
+    ms_per_step = total_ms_max / steps
+    return {"ms_per_step": ms_per_step,
+            "value": ms_per_step * 1e6 / attempts_all,                # ns per photon per attempted RK step
+            "ns_per_photon_per_accepted_step": ms_per_step * 1e6 / accepts_all,
+            "images_per_s": world / (ms_per_step * 1e-3)}
+
+
+# ---------------------------------------------------------------------------------------------------
 # the B200 arm
 # ---------------------------------------------------------------------------------------------------
 def run_b200(args):
@@ -267,20 +293,15 @@ def run_b200(args):
         e2e = (e2e_s, d2h, h2d, int(host["n_attempt"].astype("int64").sum()))
 
     # ---- reduce over ranks: time = max, work = sum
-    t = torch.tensor([total_ms, e2e[0] if e2e else 0.0], dtype=torch.float64, device="cuda")
-    n = torch.tensor([attempts, accepts, rays, launches], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(n, op=dist.ReduceOp.SUM)
-    total_ms_max, e2e_s_max = t.tolist()
-    attempts_all, accepts_all, rays_all, launches_all = n.tolist()
+    (total_ms_max, e2e_s_max), (attempts_all, accepts_all, rays_all, launches_all) = reduce_over_ranks(
+        dist, "cuda", [total_ms, e2e[0] if e2e else 0.0], [attempts, accepts, rays, launches])
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
         return 0
 
-    ms_per_step = total_ms_max / args.steps
-    value = ms_per_step * 1e6 / attempts_all                          # ns per photon per attempted RK step
+    head = headline(total_ms_max, args.steps, attempts_all, accepts_all, world)
+    ms_per_step, value = head["ms_per_step"], head["value"]
     flop_rt = FLOP_PER_RT_UPDATE if args.model == "riaf" else 0.0
     flop_step = FLOP_PER_ATTEMPT_GEODESIC * attempts + flop_rt * accepts                # per launch (this rank)
     kernel_ms = sum(step_ms) / len(step_ms)
@@ -296,8 +317,8 @@ def run_b200(args):
                    "l2": "no input arrays (rays are generated from the pixel index); the %d MB of per-step "
                          "outputs exceed the 126 MB L2" % (out_bytes >> 20),
                    "parallelism": "replicas" if world > 1 else "single GPU"},
-        "images_per_s": world / (ms_per_step * 1e-3),
-        "ns_per_photon_per_accepted_step": ms_per_step * 1e6 / accepts_all,
+        "images_per_s": head["images_per_s"],
+        "ns_per_photon_per_accepted_step": head["ns_per_photon_per_accepted_step"],
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                      "frac": achieved / peak_tflops, "traffic": None,
                      "kernel": "odyssey_kernel<KIND=%d,TAB=0,SPEC=false>" % mo["kind"], "kernel_ms": kernel_ms,
