@@ -141,7 +141,7 @@ int odyssey_kernel_info(int kind, int spectrum, int tableau, int32_t* regs, int3
 
 /* Diagnostic: evaluate one of the kernels' own FP64 elementary functions (csrc/dmath.cuh) elementwise on
  * n DEVICE doubles: op 0 1/x, 1 x^-1/2, 2 sqrt, 3 sincos (y = sin, y2 = cos), 4 exp, 5 expm1, 6 log,
- * 7 K_2(x) of eq. (37).  y2 may be NULL except for op 3.  Used by the tests to check the
+ * 7 K_2(x) of eq. (37), 8 / 9 the raw hardware seeds of 1/x and x^-1/2.  y2 may be NULL except for op 3.  Used by the tests to check the
  * device arithmetic against libm / scipy on its own, apart from the ray-level parity tests.       */
 int odyssey_eval_math(int op, int n, const double* x, double* y, double* y2, void* cuda_stream);
 

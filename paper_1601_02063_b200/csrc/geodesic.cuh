@@ -30,10 +30,12 @@ __device__ __forceinline__ void geodesic_rhs(const double a, const double a2, co
     d_sincos(th, s, c);
     sin_th = s; cos_th = c;
     if (fabs(s) < 1e-8) s = copysign(1e-8, s);
+    // 37 FP64 operations + three reciprocals (was 43): shared sub-expressions r² + a², 2q + G/Σ
     const double r2 = r * r;
+    const double ra2 = r2 + a2;                                   // r² + a²
     const double Sigma = fma(a2, c * c, r2);                      // Σ = r² + a² cos²θ
-    const double Delta = fma(r, r - 2.0, a2);                     // Δ = r² − 2r + a²
-    const double Pm = r2 + fma(a, L, a2);                         // −P
+    const double Delta = fma(-2.0, r, ra2);                       // Δ = r² − 2r + a²
+    const double Pm = fma(a, L, ra2);                             // −P = r² + a² + aL  (E = −1)
     const double iS = d_rcp(Sigma), iD = d_rcp(Delta), is = d_rcp(s);   // three independent Newton chains
     const double is2 = is * is;
     const double D = fma(L, is, a * s);                           // L/sinθ − aE sinθ
@@ -43,9 +45,9 @@ __device__ __forceinline__ void geodesic_rhs(const double a, const double a2, co
     const double GiS = G * iS;
     k.r = Delta * pr * iS;                                        // eq. (4)
     k.th = pth * iS;                                              // eq. (5)
-    k.ph = fma((Sigma - 2.0 * r) * L, is2, -2.0 * a * r) * iS * iD;   // eq. (12)
-    k.pr = iS * (fma(r, GiS, 2.0 * r * q) - (r - 1.0) * fma(q, q, pr2));
-    k.pth = s * c * iS * (fma(L * L, is2 * is2, -a2) - a2 * GiS);
+    k.ph = fma(fma(-2.0, r, Sigma) * L, is2, -2.0 * a * r) * (iS * iD);   // eq. (12)
+    k.pr = iS * fma(1.0 - r, fma(q, q, pr2), r * fma(2.0, q, GiS));
+    k.pth = (s * c) * iS * fma(-a2, GiS, fma(L * L, is2 * is2, -a2));
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -332,8 +332,8 @@ int odyssey_fp64_peak_probe(int iters, double* sink, double* flop_host, void* cu
 }
 
 int odyssey_eval_math(int op, int n, const double* x, double* y, double* y2, void* cuda_stream) {
-    if (op < 0 || op > 7 || n < 0 || (n > 0 && (!x || !y)) || (op == 3 && !y2))
-        return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "eval_math: op in [0,7], n >= 0, x and y non-NULL (y2 too for op 3)");
+    if (op < 0 || op > 9 || n < 0 || (n > 0 && (!x || !y)) || (op == 3 && !y2))
+        return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "eval_math: op in [0,9], n >= 0, x and y non-NULL (y2 too for op 3)");
     if (n == 0) return ODYSSEY_OK;
     DevState* D = nullptr;
     TRY(device_state(&D, nullptr));

@@ -329,6 +329,8 @@ __global__ void eval_math_kernel(int op, int n, const double* __restrict__ x, do
         case 4: r = d_exp(v); break;
         case 5: r = d_expm1(v); break;
         case 6: r = d_log(v); break;
+        case 8: r = d_rcp_seed(v); break;
+        case 9: r = d_rsqrt_seed(v); break;
         default: { double kf, ke; bessel_k2_inv(v, d_log(v), kf, ke); r = d_rcp(kf) * d_exp(-ke); }
     }
     y[i] = r;
