@@ -57,7 +57,8 @@ __device__ __forceinline__ bool flow_igamma(const Params& P, const double L, con
     }
     const double N = -(g_tt + 2.0 * Omega * g_tp + Omega * Omega * g_pp);
     if (!(N > 0.0)) return false;
-    const double ut = d_sqrt(1.0 + ur2_grr) * d_rsqrt(N);
+    double ut = d_rsqrt(N);
+    if (ur2_grr > 0.0) ut *= d_sqrt(1.0 + ur2_grr);                              // plunging region only
     igam = fma(ut, fma(L, Omega, 1.0), pr * ur);
     return true;
 }
