@@ -38,12 +38,13 @@ UNIT = "ns/photon/step"
 # FP64 work per unit: flop per attempted RK step of the geodesic system, and per
 # radiative-transfer update (one per accepted step, single frequency).  These are the flop the kernels
 # EXECUTE (2 x DFMA + DMUL + DADD thread instructions, predicated on), measured with ncu on this very
-# workload — profiles/r01_c4_geodesic_kernel_ncu_full.md: 1031.8 per attempt; profiles/
-# r01_c4_riaf_kernel_ncu_full.md: 1391.9 per attempt with 0.7938 accepted steps per attempt
-# -> (1391.9 - 1031.8)/0.7938 = 453.7 per update.  SURVEY.md §8(d)'s a-priori hand count (1500 + ~490)
-# is 40 % higher: it would overstate the achieved rate, so it is not used.
-FLOP_PER_ATTEMPT_GEODESIC = 1031.8
-FLOP_PER_RT_UPDATE = 453.7
+# workload — profiles/r01_c4_geodesic_kernel_ncu_full.md: 946.6 per attempt; profiles/
+# r01_c4_riaf_kernel_ncu_full.md: 1262.0 per attempt with 0.7938 accepted steps per attempt
+# -> (1262.0 - 946.6)/0.7938 = 397.3 per update.  SURVEY.md §8(d)'s a-priori hand count (1500 + ~490)
+# is 58 % higher: it would overstate the achieved rate, so it is not used.  Re-measure when the
+# kernels' arithmetic changes.
+FLOP_PER_ATTEMPT_GEODESIC = 946.6
+FLOP_PER_RT_UPDATE = 397.3
 
 
 def parse_args():
