@@ -13,11 +13,11 @@
 // product is assembled in log space and exponentiated ONCE per frequency:
 //   ε = r_g j_coef ν_0 n_e M(x_M) / (K_2(1/Θ_e) γ ν_0³)
 //     = r_g · Kfac · u² (1 + 0.40 u³ + 0.5316 u⁶) · exp( E + c_k − 1.8899 t⁴ ),
-//   t = x_M^(1/12) = exp((ln ν_k + ln(1/γ) − ln ν_c)/12),  u = 1/t,   (eq. (38): x^1/6 = t², x^1/4 = t³, x^1/3 = t⁴)
+//   t = x_M^(1/12) = ν_k^(1/12) · exp((ln(1/γ) − ln ν_c)/12),  u = 1/t,   (eq. (38): x^1/6 = t², x^1/4 = t³, x^1/3 = t⁴)
 //   E = ln(4.0505 j_coef) + ln n_e + Kexp − ln(1/γ),  c_k = −2 ln ν_k,  1/K_2 = Kfac · e^Kexp,
 //   a = ε · expm1(h ν_0 / k T_e) · c²/(2h)                              (Kirchhoff with B_ν0(T_e)),
 // with ln n_e, ln Θ_e, ln ν_c linear in ln r, cos²θ and constants.  Per point this needs two logarithms
-// (ln r, ln 1/γ) and one exponential (1/Θ_e); per frequency two exponentials and one expm1, instead of
+// (ln r, ln 1/γ) and two exponentials (1/Θ_e, t/ν^(1/12)); per frequency one exponential and one expm1, instead of
 // the dozen pow/exp/cbrt/sqrt/divisions of the formulas as printed.  Same mathematics, different
 // rounding (parity tolerance on images: 1e-6 relative L1).
 #pragma once
@@ -98,13 +98,13 @@ struct RtPoint {
     bool on;            // inside the emitting region with a valid flow
     double fac;         // r_g · Kfac
     double E;           // exponent shared by all frequencies
-    double lxm0;        // ln x_M − ln ν = ln(1/γ) − ln ν_c
+    double t0, u0;      // (x_M / ν)^(1/12) and its reciprocal: x_M^(1/12) = t0 ν^(1/12)
     double ycoef;       // h ν_0 /(k T_e) = ν · ycoef
 };
 
 __device__ __forceinline__ void rt_point(const Params& P, const double L, const double r, const double s, const double c,
                                          const double pr, RtPoint& q) {
-    q.on = false; q.fac = 0.0; q.E = 0.0; q.lxm0 = 0.0; q.ycoef = 0.0;     // off: every coefficient evaluates to 0
+    q.on = false; q.fac = 0.0; q.E = 0.0; q.t0 = 1.0; q.u0 = 1.0; q.ycoef = 0.0;   // off: every coefficient evaluates to 0
     if (!(r > P.r_cap && r < P.r_rt_out)) return;
     double igam;
     if (!flow_igamma(P, L, r, s, c, pr, igam)) return;
@@ -124,17 +124,18 @@ __device__ __forceinline__ void rt_point(const Params& P, const double L, const 
     q.on = true;
     q.fac = P.rg_cm * kfac;
     q.E = P.ln_j0 + ln_ne + kexp - ligam;
-    q.lxm0 = ligam - ln_nuc;
+    q.t0 = d_exp_nc((ligam - ln_nuc) * (1.0 / 12.0));               // ln(x_M/ν) = ln(1/γ) − ln ν_c; |argument| < 700
+    q.u0 = d_rcp(q.t0);
     q.ycoef = P.h_over_mc2 * igam * x;
 }
 
 // Per-frequency coefficients.  ln_nu = ln ν_k.
-__device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& q, const double nu, const double ln_nu,
-                                                double& acoef, double& ecoef) {
+__device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& q, const int k, double& acoef, double& ecoef) {
+    const double nu = P.nu[k], ln_nu = P.ln_nu[k];
     // straight-line on purpose (no early return when the point is off: fac = 0 gives ε = a = 0), so that the
     // spectrum kernel's unrolled frequency loop can interleave independent chains
-    const double t = d_exp_nc((ln_nu + q.lxm0) * (1.0 / 12.0));     // x_M^(1/12); |argument| < 700 always
-    const double u = d_rcp(t);
+    const double t = q.t0 * P.nu12[k];                               // x_M^(1/12)
+    const double u = q.u0 * P.inu12[k];
     const double t2 = t * t, u2 = u * u;
     const double u3 = u2 * u;
     const double poly = fma(u3, fma(0.5316, u3, 0.40), 1.0);        // eq. (38) bracket

@@ -146,7 +146,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
         P->r_rt_out = M->r_rt_out; P->tau_max = M->tau_max;
         P->rg_cm = kGMsun * M->mbh_msun / (kC * kC);
         P->sed_coef = 4.0 * kPi * P->rg_cm * P->rg_cm * P->pix_area;
-        for (int k = 0; k < nf && k < MAX_FREQ; ++k) { P->nu[k] = nu[k]; P->ln_nu[k] = std::log(nu[k]); P->nu3[k] = nu[k] * nu[k] * nu[k]; }
+        for (int k = 0; k < nf && k < MAX_FREQ; ++k) { P->nu[k] = nu[k]; P->ln_nu[k] = std::log(nu[k]); P->nu12[k] = std::exp(P->ln_nu[k] / 12.0); P->inu12[k] = 1.0 / P->nu12[k]; P->nu3[k] = nu[k] * nu[k] * nu[k]; }
     }
 }
 

@@ -240,14 +240,14 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     // unrolled iterations are independent chains the scheduler can interleave
                     double tk = ACC(0, k), Tk = ACC(1, k), Ik = ACC(2, k);
                     const double a0k = ACC(3, k), e0k = ACC(4, k);
-                    double a1, e1; rt_coefficients(P, pt, P.nu[k], P.ln_nu[k], a1, e1);
+                    double a1, e1; rt_coefficients(P, pt, k, a1, e1);
                     rt_update(a0k, a1, e0k, e1, commit ? h_try : 0.0, P.tau_max, tk, Tk, Ik);   // fresh lane: zero-length step
                     ACC(0, k) = tk; ACC(1, k) = Tk; ACC(2, k) = Ik;
                     if (!(tk > P.tau_max)) all_opaque = false;
                     ACC(3, k) = a1; ACC(4, k) = e1;
                 }
             } else {
-                double a1, e1; rt_coefficients(P, pt, P.nu[0], P.ln_nu[0], a1, e1);
+                double a1, e1; rt_coefficients(P, pt, 0, a1, e1);
                 if (commit) {
                     double tau = RT1(0), Tr = RT1(1), Inu = RT1(2);
                     rt_update(RT1(3), a1, RT1(4), e1, h_try, P.tau_max, tau, Tr, Inu);

@@ -40,6 +40,7 @@ struct Params {
     int32_t nf, pad;
     double nu[MAX_FREQ];
     double ln_nu[MAX_FREQ];
+    double nu12[MAX_FREQ], inu12[MAX_FREQ];     // ν^(1/12) and its reciprocal (eq. (38) in powers of x_M^(1/12))
     double nu3[MAX_FREQ];                       // ν^3 (observed), image = ν^3 × invariant intensity
 };
 
