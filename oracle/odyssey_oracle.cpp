@@ -25,7 +25,8 @@
 // the null condition; capture classification vs the closed-form radial potential; shadow edges
 // sqrt(27) and Bardeen's xi(r_ph); Schwarzschild deflection vs quadrature; an independent
 // 8-component scipy integration of Hamilton's equations (E, L_z drift there); closed-form Keplerian
-// g; uniform-slab RT; K_2 vs scipy; M(1) as printed in eq. (38).
+// g; uniform-slab RT; the thin limit and the formal solution int eps e^-tau dlambda by independent
+// quadrature on a finer path; K_2 vs scipy; M(1) as printed in eq. (38).
 // PARITY UNPINNED: the RIAF images and the SED as a whole (oracle_render_image kind 2,
 // oracle_render_spectrum) have no value printed in the paper to compare with (Figs. 9, 10 are
 // pictures, Broderick & Loeb's table is not in the container); their parts are pinned, the whole
