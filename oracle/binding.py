@@ -30,7 +30,8 @@ class Model(C.Structure):
                 ("mbh_msun", C.c_double), ("n0", C.c_double), ("n_index", C.c_double), ("T0", C.c_double),
                 ("T_index", C.c_double), ("h_over_r", C.c_double), ("beta", C.c_double),
                 ("r_rt_out", C.c_double), ("tau_max", C.c_double), ("j_scale", C.c_double),
-                ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double)]
+                ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double),
+                ("rt_scheme", C.c_int32), ("pad", C.c_int32)]
 
 
 def _fill(struct, d):
@@ -176,6 +177,12 @@ def rt_update(a0, a1, e0, e1, dl, tau_max, tau, T, I):
     lib().oracle_rt_update(C.c_double(a0), C.c_double(a1), C.c_double(e0), C.c_double(e1), C.c_double(dl),
                            C.c_double(tau_max), _dp(st))
     return st[0], st[1], st[2]
+
+
+def rt_rk_step(which, a, eps, h, tau_max, tau, I):
+    st = np.array([tau, I], dtype=np.float64)
+    lib().oracle_rt_rk_step(C.c_int(which), _dp(_vec(a)), _dp(_vec(eps)), C.c_double(h), C.c_double(tau_max), _dp(st))
+    return float(st[0]), float(st[1])
 
 
 def trace_points(scene, model, nu, xs, ys):

@@ -74,6 +74,7 @@ struct Model {           // mirrors workloads.model_*()
     double r_in, r_out, emis_index;
     double mbh_msun, n0, n_index, T0, T_index, h_over_r, beta, r_rt_out, tau_max, j_scale;
     double g_lo, g_hi, g_power;
+    int32_t rt_scheme, pad;  // 0: one update per accepted step [reading E]; 1: tau, I as Runge-Kutta components [E']
 };
 
 // ----------------------------------------------------------------------------------------------
@@ -225,13 +226,16 @@ Tableau make_tableau(int which) {
 
 // One attempt of size h from y: 5th-order result ynew and the error estimate yerr = 5th - 4th,
 // formed as h * sum (b5_j - b4_j) k_j exactly as Press et al.'s rkck does.
-void rk_attempt(const Ray& ray, const Tableau& T, const double y[5], double h, double ynew[5], double yerr[5]) {
+// ystage (optional) receives the six stage states y + h sum_j A_ij k_j.
+void rk_attempt(const Ray& ray, const Tableau& T, const double y[5], double h, double ynew[5], double yerr[5],
+                double (*ystage)[5] = nullptr) {
     double k[6][5], ytmp[5];
     for (int i = 0; i < 6; ++i) {
         for (int v = 0; v < 5; ++v) {
             double acc = 0.0;
             for (int j = 0; j < i; ++j) acc += T.A[i][j] * k[j][v];
             ytmp[v] = y[v] + h * acc;
+            if (ystage) ystage[i][v] = ytmp[v];
         }
         rhs(ray, ytmp, k[i]);
     }
@@ -385,6 +389,27 @@ void rt_update(double a0, double a1, double e0, double e1, double dl, double tau
     *tau += dtau;
 }
 
+// Alternative reading [E'] of PAPER.md:L171 ("easily integrated along with the geodesic"): tau and the
+// invariant intensity are two more components of the Runge-Kutta system,
+//   dtau/dlambda = a(lambda),   dI/dlambda = eps(lambda) exp(-tau(lambda))      (eqs. (30), (31)),
+// advanced through the same six stages with the fifth-order weights; they do not enter the error norm
+// (the geodesic alone controls the step, so both schemes take identical steps).  a[i], eps[i] are the
+// coefficients at the six stage states.  A frequency is frozen once tau > tau_max, as in rt_update.
+void rt_rk_step(const Tableau& T, const double a[6], const double eps[6], double h, double tau_max,
+                double* tau, double* I) {
+    if (*tau > tau_max) return;
+    double s_tau = 0.0, s_I = 0.0;
+    for (int i = 0; i < 6; ++i) {
+        double acc = 0.0;
+        for (int j = 0; j < i; ++j) acc += T.A[i][j] * a[j];
+        double tau_i = *tau + h * acc;                     // stage value of tau
+        s_tau += T.b5[i] * a[i];
+        s_I += T.b5[i] * eps[i] * std::exp(-tau_i);
+    }
+    *I += h * s_I;
+    *tau += h * s_tau;
+}
+
 // ----------------------------------------------------------------------------------------------
 // Step 8 + the per-ray driver.
 // ----------------------------------------------------------------------------------------------
@@ -417,8 +442,8 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
 
     while (flag < 0) {
         if (n_attempt >= S.max_attempts) { flag = MAXSTEP; break; }
-        double ynew[5], yerr[5];
-        rk_attempt(ray, T, y, h, ynew, yerr);
+        double ynew[5], yerr[5], ystage[6][5];
+        rk_attempt(ray, T, y, h, ynew, yerr, ystage);
         ++n_attempt;
         double err = error_norm(y, yerr, S.rtol);
         if (!(err <= 1.0)) {                               // reject (also when err is NaN)
@@ -440,7 +465,7 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
                 double dy[5];
                 rhs(ray, ynew, dy);
                 h_used -= f / dy[comp];
-                rk_attempt(ray, T, y, h_used, ynew, yerr);
+                rk_attempt(ray, T, y, h_used, ynew, yerr, ystage);
                 ++n_attempt;
             }
         };
@@ -465,7 +490,7 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
             else if (ynew[3] > 0.0 && ynew[0] >= S.r_esc) { locate(0, S.r_esc); flag = ESCAPED; }
         }
         // RT over the step actually taken
-        if (M.kind == 2) {
+        if (M.kind == 2 && M.rt_scheme == 0) {
             rt_coefficients(S, M, F, ray, ynew, nf, nu, a1.data(), e1.data());
             bool all_opaque = true;
             for (int k = 0; k < nf; ++k) {
@@ -473,6 +498,18 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
                 if (!(tau[k] > M.tau_max)) all_opaque = false;
             }
             a0.swap(a1); e0.swap(e1);
+            if (flag < 0 && all_opaque) flag = OPAQUE;
+        } else if (M.kind == 2) {                       // [E']: coefficients at the six stage states of the step taken
+            std::vector<double> as(6 * (size_t)nf), es(6 * (size_t)nf);
+            for (int i = 0; i < 6; ++i)
+                rt_coefficients(S, M, F, ray, ystage[i], nf, nu, &as[(size_t)i * nf], &es[(size_t)i * nf]);
+            bool all_opaque = true;
+            for (int k = 0; k < nf; ++k) {
+                double ak[6], ek[6];
+                for (int i = 0; i < 6; ++i) { ak[i] = as[(size_t)i * nf + k]; ek[i] = es[(size_t)i * nf + k]; }
+                rt_rk_step(T, ak, ek, h_used, M.tau_max, &tau[k], &I[k]);
+                if (!(tau[k] > M.tau_max)) all_opaque = false;
+            }
             if (flag < 0 && all_opaque) flag = OPAQUE;
         }
         for (int v = 0; v < 5; ++v) y[v] = ynew[v];
@@ -589,6 +626,12 @@ void oracle_synchrotron(const Model* M, double a, double r, double th, double nu
 // state = {tau, T, I}, updated in place
 void oracle_rt_update(double a0, double a1, double e0, double e1, double dl, double tau_max, double* state) {
     rt_update(a0, a1, e0, e1, dl, tau_max, &state[0], &state[1], &state[2]);
+}
+
+// a[6], eps[6]: coefficients at the six stages; state = {tau, I}, updated in place [reading E']
+void oracle_rt_rk_step(int which, const double* a, const double* eps, double h, double tau_max, double* state) {
+    Tableau T = make_tableau(which);
+    rt_rk_step(T, a, eps, h, tau_max, &state[0], &state[1]);
 }
 
 // Trace n rays that start at arbitrary image-plane points (xs[k], ys[k]).  Any output may be NULL.

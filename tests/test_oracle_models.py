@@ -292,3 +292,57 @@ def test_riaf_image_converges_under_rtol_refinement():
     d2 = np.abs(imgs[1] - imgs[2]).sum() / imgs[2].sum()
     assert d2 < d1 < 0.05
     assert d2 < 5e-3
+
+
+# ---- reading E': tau and I as Runge-Kutta components (workloads.RT_RK_COMPONENTS) ---------------------
+@pytest.mark.parametrize("which", [W.TABLEAU_RKF45, W.TABLEAU_CASH_KARP])
+def test_rt_rk_step_constant_coefficients_closed_form_and_order(which):
+    """Constant a, eps over a step: tau grows linearly (exact), I = eps e^-tau0 (1 - e^-(a h))/a up to the
+    fifth-order quadrature error, which falls by ~2^6 per halving of h (local error O(h^6))."""
+    c, _, _, _ = O.tableau(which)
+    a, eps, tau0, I0 = 0.7, 3.0, 0.4, 1.25
+    errs = []
+    for h in (0.8, 0.4, 0.2):
+        tau, I = O.rt_rk_step(which, [a] * 6, [eps] * 6, h, 30.0, tau0, I0)
+        assert tau == pytest.approx(tau0 + a * h, rel=1e-15)
+        exact = I0 + eps * math.exp(-tau0) * (1.0 - math.exp(-a * h)) / a
+        errs.append(abs(I - exact))
+    assert errs[0] < 5e-6
+    assert 40 < errs[0] / errs[1] < 100 and 40 < errs[1] / errs[2] < 100
+    # stage abscissae enter through the stage values of tau: a linear-in-lambda absorption a(l) = a0 + s l
+    s, h = 0.5, 0.3
+    tau, _ = O.rt_rk_step(which, [a + s * ci * h for ci in c], [0.0] * 6, h, 30.0, 0.0, 0.0)
+    assert tau == pytest.approx(a * h + 0.5 * s * h * h, rel=1e-14)
+    # frozen once tau > tau_max
+    assert O.rt_rk_step(which, [1.0] * 6, [1.0] * 6, 1.0, 30.0, 30.5, 7.0) == (30.5, 7.0)
+
+
+def test_rk_component_scheme_along_a_ray_equals_formal_solution():
+    """Same ray and frequency as the per-step pin above; the Runge-Kutta-component scheme is of higher
+    order in the step, so it sits closer to the fine-path formal solution than the per-step scheme."""
+    a, nu = 0.9375, 30e9
+    sc = W.scene(a, 30.0, 64, 15.0, rtol=1e-9)
+    x, y = 5.0, 2.0
+    I0 = O.trace_points(sc, W.model_riaf(), [nu], [x], [y])
+    I1 = O.trace_points(sc, W.model_riaf(rt_scheme=W.RT_RK_COMPONENTS), [nu], [x], [y])
+    fine = O.trace_points(dict(sc, rtol=1e-13), W.model_riaf(rt_scheme=W.RT_RK_COMPONENTS), [nu], [x], [y])
+    assert I1["n_attempt"][0] == I0["n_attempt"][0]                # the geodesic alone controls the steps
+    assert I1["tau"][0, 0] == pytest.approx(fine["tau"][0, 0], rel=1e-5)
+    assert I1["I"][0, 0] == pytest.approx(fine["I"][0, 0], rel=1e-4)
+    assert abs(I1["I"][0, 0] - fine["I"][0, 0]) < abs(I0["I"][0, 0] - fine["I"][0, 0])
+    assert I0["I"][0, 0] == pytest.approx(fine["I"][0, 0], rel=5e-3)
+
+
+def test_the_two_transfer_schemes_converge_to_the_same_image():
+    """Cross-pin for the RIAF image as a whole (no printed value exists): two different discretisations
+    of eqs. (30), (31) along identical geodesics approach each other as the tolerance is refined."""
+    w = W.C2(n=16)
+    d = []
+    for rtol in (1e-6, 1e-8, 1e-10):
+        sc = dict(w["scene"], rtol=rtol)
+        a = O.render_image(sc, w["model"], w["nu"][0])
+        b = O.render_image(sc, dict(w["model"], rt_scheme=W.RT_RK_COMPONENTS), w["nu"][0])
+        assert np.array_equal(a["flag"], b["flag"]) and np.array_equal(a["n_attempt"], b["n_attempt"])
+        d.append(np.abs(a["image"] - b["image"]).sum() / a["image"].sum())
+    assert d[0] > d[1] > d[2]
+    assert d[2] < 2e-4

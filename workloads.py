@@ -19,6 +19,9 @@ import math
 FLAG_ESCAPED, FLAG_CAPTURED, FLAG_DISK, FLAG_OPAQUE, FLAG_MAXSTEP = 0, 1, 2, 3, 4
 
 KIND_NONE, KIND_THIN_DISK, KIND_RIAF = 0, 1, 2
+# How eqs. (30), (31) are advanced (readings E, E'): one exact-attenuation update per accepted
+# step (default), or tau and I as two more Runge-Kutta components through the six stages.
+RT_PER_STEP, RT_RK_COMPONENTS = 0, 1
 TABLEAU_RKF45, TABLEAU_CASH_KARP = 0, 1
 
 
@@ -37,7 +40,7 @@ def model_none():
     return dict(kind=KIND_NONE, r_in=0.0, r_out=0.0, emis_index=0.0,
                 mbh_msun=0.0, n0=0.0, n_index=0.0, T0=0.0, T_index=0.0, h_over_r=1.0, beta=1.0,
                 r_rt_out=0.0, tau_max=0.0, j_scale=1.0,
-                nbins=0, g_lo=0.0, g_hi=1.0, g_power=0.0)
+                nbins=0, g_lo=0.0, g_hi=1.0, g_power=0.0, rt_scheme=RT_PER_STEP)
 
 
 def model_thin_disk(r_in=0.0, r_out=50.0, emis_index=3.0, nbins=200, g_lo=0.0, g_hi=2.0, g_power=3.0):
@@ -50,12 +53,12 @@ def model_thin_disk(r_in=0.0, r_out=50.0, emis_index=3.0, nbins=200, g_lo=0.0, g
 
 
 def model_riaf(mbh_msun=4.0e6, n0=1.0e7, n_index=-1.1, T0=1.0e11, T_index=-0.84, h_over_r=0.3,
-               beta=10.0, r_rt_out=500.0, tau_max=30.0, j_scale=1.0):
+               beta=10.0, r_rt_out=500.0, tau_max=30.0, j_scale=1.0, rt_scheme=RT_PER_STEP):
     """Analytic RIAF-like flow of BASELINE.json:configs[2]; mass and outer radius from PAPER.md:L292."""
     m = model_none()
     m.update(kind=KIND_RIAF, mbh_msun=float(mbh_msun), n0=float(n0), n_index=float(n_index),
              T0=float(T0), T_index=float(T_index), h_over_r=float(h_over_r), beta=float(beta),
-             r_rt_out=float(r_rt_out), tau_max=float(tau_max), j_scale=float(j_scale))
+             r_rt_out=float(r_rt_out), tau_max=float(tau_max), j_scale=float(j_scale), rt_scheme=int(rt_scheme))
     return m
 
 
