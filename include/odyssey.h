@@ -55,6 +55,12 @@ enum {
 
 enum { ODYSSEY_TABLEAU_RKF45 = 0, ODYSSEY_TABLEAU_CASH_KARP = 1 };
 enum { ODYSSEY_KIND_NONE = 0, ODYSSEY_KIND_THIN_DISK = 1, ODYSSEY_KIND_RIAF = 2 };
+/* PAPER.md:L171 says the transfer equations are "easily integrated along with the geodesic … piecewise
+ * according to these steps".  PER_STEP (default): one update per accepted step, trapezoid in lambda with
+ * the exact attenuation across the step.  RK_COMPONENTS: tau and I as two more components of the
+ * Runge–Kutta system (coefficients evaluated at all six stages, fifth-order weights, not in the error
+ * norm); single-frequency calls only.                                                              */
+enum { ODYSSEY_RT_PER_STEP = 0, ODYSSEY_RT_RK_COMPONENTS = 1 };
 #define ODYSSEY_MAX_FREQ 32
 
 /* The observer, the image plane and the integrator controls. */
@@ -87,6 +93,8 @@ typedef struct odyssey_model {
     double j_scale;            /* kind 2: 1 = per-steradian emissivity; 4π reproduces eq. (37) as printed */
     double g_lo, g_hi;         /* kind 1: histogram range in g                                   */
     double g_power;            /* kind 1: pixel value = g^g_power r_e^-emis_index                */
+    int32_t rt_scheme;         /* kind 2: ODYSSEY_RT_* — how eqs. (30), (31) are advanced along the ray */
+    int32_t pad2;
 } odyssey_model;
 
 /* Geodesics only (BASELINE.json:configs[0]; §2.1-2.2).  Per pixel: outcome flag, the

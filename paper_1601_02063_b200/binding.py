@@ -42,7 +42,8 @@ class Model(C.Structure):
                 ("mbh_msun", C.c_double), ("n0", C.c_double), ("n_index", C.c_double),
                 ("T0", C.c_double), ("T_index", C.c_double), ("h_over_r", C.c_double), ("beta", C.c_double),
                 ("r_rt_out", C.c_double), ("tau_max", C.c_double), ("j_scale", C.c_double),
-                ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double)]
+                ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double),
+                ("rt_scheme", C.c_int32), ("pad2", C.c_int32)]
 
 
 def _struct(cls, d):

@@ -98,13 +98,17 @@ struct RtPoint {
     bool on;            // inside the emitting region with a valid flow
     double fac;         // r_g · Kfac
     double E;           // exponent shared by all frequencies
-    double t0, u0;      // (x_M / ν)^(1/12) and its reciprocal: x_M^(1/12) = t0 ν^(1/12)
+    double t0, u0;      // spectrum kernel: (x_M / ν)^(1/12) and its reciprocal, x_M^(1/12) = t0 ν^(1/12)
+    double lxm0;        // single-frequency kernels: ln(x_M / ν) = ln(1/γ) − ln ν_c
     double ycoef;       // h ν_0 /(k T_e) = ν · ycoef
 };
 
+// HOIST: evaluate the x_M^(1/12) exponential once per point (spectrum kernel: ν_k^(1/12) is a constant per
+// frequency) instead of once per frequency (single-frequency kernels: same work, fewer live registers).
+template <bool HOIST>
 __device__ __forceinline__ void rt_point(const Params& P, const double L, const double r, const double s, const double c,
                                          const double pr, RtPoint& q) {
-    q.on = false; q.fac = 0.0; q.E = 0.0; q.t0 = 1.0; q.u0 = 1.0; q.ycoef = 0.0;   // off: every coefficient evaluates to 0
+    q.on = false; q.fac = 0.0; q.E = 0.0; q.t0 = 1.0; q.u0 = 1.0; q.lxm0 = 0.0; q.ycoef = 0.0;   // off: every coefficient evaluates to 0
     if (!(r > P.r_cap && r < P.r_rt_out)) return;
     double igam;
     if (!flow_igamma(P, L, r, s, c, pr, igam)) return;
@@ -124,18 +128,24 @@ __device__ __forceinline__ void rt_point(const Params& P, const double L, const 
     q.on = true;
     q.fac = P.rg_cm * kfac;
     q.E = P.ln_j0 + ln_ne + kexp - ligam;
-    q.t0 = d_exp_nc((ligam - ln_nuc) * (1.0 / 12.0));               // ln(x_M/ν) = ln(1/γ) − ln ν_c; |argument| < 700
-    q.u0 = d_rcp(q.t0);
+    if (HOIST) {
+        q.t0 = d_exp_nc((ligam - ln_nuc) * (1.0 / 12.0));           // ln(x_M/ν) = ln(1/γ) − ln ν_c; |argument| < 700
+        q.u0 = d_rcp(q.t0);
+    } else {
+        q.lxm0 = ligam - ln_nuc;
+    }
     q.ycoef = P.h_over_mc2 * igam * x;
 }
 
 // Per-frequency coefficients.  ln_nu = ln ν_k.
+template <bool HOIST>
 __device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& q, const int k, double& acoef, double& ecoef) {
     const double nu = P.nu[k], ln_nu = P.ln_nu[k];
     // straight-line on purpose (no early return when the point is off: fac = 0 gives ε = a = 0), so that the
     // spectrum kernel's unrolled frequency loop can interleave independent chains
-    const double t = q.t0 * P.nu12[k];                               // x_M^(1/12)
-    const double u = q.u0 * P.inu12[k];
+    double t, u;                                                     // x_M^(1/12) and its reciprocal
+    if (HOIST) { t = q.t0 * P.nu12[k]; u = q.u0 * P.inu12[k]; }
+    else { t = d_exp_nc((ln_nu + q.lxm0) * (1.0 / 12.0)); u = d_rcp(t); }
     const double t2 = t * t, u2 = u * u;
     const double u3 = u2 * u;
     const double poly = fma(u3, fma(0.5316, u3, 0.40), 1.0);        // eq. (38) bracket

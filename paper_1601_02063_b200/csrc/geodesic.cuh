@@ -125,6 +125,7 @@ __constant__ double kRkBE[2][6] = { ODY_BE(0), ODY_BE(1) };
 // They live in shared memory, [component][stage][thread] — consecutive lanes hit consecutive 8-byte
 // words, so every access is conflict-free.  This takes 48 registers off the kernel, which is what lets
 // it run 5 blocks of 128 threads per SM at 96 registers without spills.
+constexpr int STAGE_ROWS = 5;                           // r, θ, p_r, p_θ slopes + the absorption coefficient (RT scheme E')
 template <int NT>
 struct StagesSmem {
     double* base;                                       // &smem[threadIdx.x]
@@ -146,6 +147,16 @@ __device__ __forceinline__ void stage_point(const KS& K, const State& y, const d
         }
     }
     r = fma(h, sr, y.r); th = fma(h, st, y.th); pr = fma(h, sp, y.pr); pth = fma(h, sq, y.pth);
+}
+
+// Σ_{j<I} a_Ij v_j of row `c` (used for the stage values of τ in the Runge–Kutta-component transfer scheme).
+template <int TAB, int I, class KS>
+__device__ __forceinline__ double stage_sum(const KS& K, const int c) {
+    double acc = 0.0;
+#pragma unroll
+    for (int j = 0; j < I; ++j)
+        if (rk_a<TAB>(I, j) != 0.0) acc = fma(kRkA[TAB][I][j], K.get(c, j), acc);
+    return acc;
 }
 
 // Fifth-order result and the error estimate h Σ (b5_j − b4_j) k_j (as Press et al.'s rkck forms it)

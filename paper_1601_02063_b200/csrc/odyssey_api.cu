@@ -95,6 +95,8 @@ int check_model(const odyssey_model* M) {
         if (M->nbins > 0 && !(M->g_hi > M->g_lo)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "g_hi must exceed g_lo");
     }
     if (M->kind == ODYSSEY_KIND_RIAF) {
+        if (M->rt_scheme != ODYSSEY_RT_PER_STEP && M->rt_scheme != ODYSSEY_RT_RK_COMPONENTS)
+            return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown rt_scheme %d", M->rt_scheme);
         if (!(M->mbh_msun > 0.0) || !(M->h_over_r > 0.0) || !(M->beta > 0.0) || !(M->T0 > 0.0) || !(M->n0 >= 0.0) ||
             !(M->j_scale >= 0.0))
             return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "RIAF parameters mbh_msun, h_over_r, beta, T0 must be positive, n0 and j_scale non-negative");
@@ -143,7 +145,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
         P->ln_j0 = std::log(4.0505 * M->j_scale * kE * kE / (std::sqrt(3.0) * kC));
         P->h_over_mc2 = kH / (kMe * kC * kC);
         P->inv_planck = kC * kC / (2.0 * kH);
-        P->r_rt_out = M->r_rt_out; P->tau_max = M->tau_max;
+        P->r_rt_out = M->r_rt_out; P->tau_max = M->tau_max; P->rt_scheme = M->rt_scheme;
         P->rg_cm = kGMsun * M->mbh_msun / (kC * kC);
         P->sed_coef = 4.0 * kPi * P->rg_cm * P->rg_cm * P->pix_area;
         for (int k = 0; k < nf && k < MAX_FREQ; ++k) { P->nu[k] = nu[k]; P->ln_nu[k] = std::log(nu[k]); P->nu12[k] = std::exp(P->ln_nu[k] / 12.0); P->inu12[k] = 1.0 / P->nu12[k]; P->nu3[k] = nu[k] * nu[k] * nu[k]; }
@@ -152,11 +154,14 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
 
 // ---- kernel table ------------------------------------------------------------------------------
 constexpr int NT_MAIN = 128, MINB_MAIN = 5;     // 96 registers per thread at most
+constexpr int MINB_RK = 2;                      // transfer scheme E' (RK components): the in-loop transfer code wants > 168 registers
 constexpr int NT_SPEC = 128, MINB_SPEC = 3;     // 168 registers (the unrolled frequency loop wants them); per-frequency accumulators in a global scratch buffer
 
 typedef void (*KernelFn)(const Params, const Outputs);
 
-KernelFn pick_kernel(int kind, bool spec, int tab) {
+KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0) {
+    if (kind == 2 && !spec && rts == 1)
+        return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_RK, 1> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_RK, 1>;
     if (spec) return tab ? odyssey_kernel<2, 1, true, NT_SPEC, MINB_SPEC> : odyssey_kernel<2, 0, true, NT_SPEC, MINB_SPEC>;
     switch (kind) {
         case 0: return tab ? odyssey_kernel<0, 1, false, NT_MAIN, MINB_MAIN> : odyssey_kernel<0, 0, false, NT_MAIN, MINB_MAIN>;
@@ -165,9 +170,9 @@ KernelFn pick_kernel(int kind, bool spec, int tab) {
     }
 }
 
-size_t smem_bytes(int kind, bool spec, int nf, int nbins) {
-    if (spec) return (size_t)(29 * NT_SPEC + MAX_FREQ) * sizeof(double);
-    const size_t stages = (size_t)29 * NT_MAIN * sizeof(double);         // [4][6][NT] stage slopes + [5][NT] RT state
+size_t smem_bytes(int kind, bool spec, int nf, int nbins, int rts = 0) {
+    if (spec) return (size_t)(smem_per_thread(0) * NT_SPEC + MAX_FREQ) * sizeof(double);
+    const size_t stages = (size_t)smem_per_thread(kind == 2 ? rts : 0) * NT_MAIN * sizeof(double);   // stage values + [5][NT] RT state
     if (kind == 1) return stages + (size_t)(nbins > 0 ? nbins : 1) * sizeof(double);
     return stages;
 }
@@ -176,9 +181,9 @@ int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
     DevState* D = nullptr;
     int rc = device_state(&D, nullptr);
     if (rc) return rc;
-    KernelFn fn = pick_kernel(P.kind, spec, tab);
+    KernelFn fn = pick_kernel(P.kind, spec, tab, P.rt_scheme);
     const int nt = spec ? NT_SPEC : NT_MAIN;
-    const size_t sm = smem_bytes(P.kind, spec, P.nf, P.nbins);
+    const size_t sm = smem_bytes(P.kind, spec, P.nf, P.nbins, P.rt_scheme);
     if (sm > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
     int per_sm = 0;
     CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fn, nt, sm));
@@ -270,6 +275,7 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
     rc = check_model(model);
     if (rc) return rc;
     if (model->kind != ODYSSEY_KIND_RIAF) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode needs model kind 2 (RIAF), got %d", model->kind);
+    if (model->rt_scheme != ODYSSEY_RT_PER_STEP) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode supports rt_scheme 0 (per-step update) only");
     if (nf < 1 || nf > ODYSSEY_MAX_FREQ) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nf = %d outside [1, %d]", nf, ODYSSEY_MAX_FREQ);
     if (!nu_hz_host) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz_host is NULL");
     for (int k = 0; k < nf; ++k)

@@ -54,18 +54,23 @@ __device__ __forceinline__ void store_stage(KS& K, const Slope& k, double& ph5, 
     if (rk_b5<TAB>(I) - rk_b4<TAB>(I) != 0.0) phe = fma(kRkBE[TAB][I], k.ph, phe);
 }
 
-template <int KIND, int TAB, bool SPEC, int NT, int MINB>
+// Shared-memory doubles per thread: rows x 6 stage values + 5 single-frequency transfer values
+// (rows = 4 slopes, + the absorption coefficient for transfer scheme E').
+__host__ __device__ constexpr int smem_per_thread(int rts) { return (rts ? STAGE_ROWS : STAGE_ROWS - 1) * 6 + 5; }
+
+// RTS = 1: transfer scheme E' (tau, I as Runge–Kutta components; single frequency only).
+template <int KIND, int TAB, bool SPEC, int NT, int MINB, int RTS = 0>
 __global__ void __launch_bounds__(NT, MINB)
 odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs O) {
     extern __shared__ double smem[];
     const int lane = threadIdx.x & 31;
     const int nf = SPEC ? P.nf : 1;
-    // shared layout: [4][6][NT] stage slopes, [5][NT] single-frequency RT state, then hist[nbins] (KIND 1)
+    // shared layout: [5][6][NT] stage values, [5][NT] single-frequency RT state, then hist[nbins] (KIND 1)
     // or sed[MAX_FREQ] (SPEC).  The spectrum variant's 5 x nf per-frequency accumulators live in a global
     // scratch buffer laid out [quantity][frequency][grid thread] (every warp access is one contiguous
     // 256-byte segment; 160 doubles per thread would cap the SM at 5 warps if they sat in shared memory).
-    double* const sm_red = smem + 29 * NT;
-    double* const sm_rt = smem + 24 * NT + threadIdx.x;            // (!SPEC) q: 0 tau, 1 T, 2 I, 3 a0, 4 e0
+    double* const sm_red = smem + smem_per_thread(RTS) * NT;
+    double* const sm_rt = smem + (smem_per_thread(RTS) - 5) * NT + threadIdx.x;            // (!SPEC) q: 0 tau, 1 T, 2 I, 3 a0, 4 e0
     const size_t spec_stride = (size_t)gridDim.x * NT;
     double* const gl_acc = SPEC ? O.spec_state + (size_t)blockIdx.x * NT + threadIdx.x : nullptr;
 #define RT1(q) sm_rt[(q) * NT]
@@ -135,6 +140,14 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         bool done = false;                                             // end state evaluated: go on to events / commit
         double ph5 = kRkB5[TAB][0] * kph0;
         double phe = kRkBE[TAB][0] * kph0;
+        // scheme E': running fifth-order sums of a and of eps exp(-tau) over the stages; stage 0 = cached start values
+        double rk_tau = 0.0, rk_I = 0.0, tau_n = 0.0;
+        if (RTS == 1) {
+            tau_n = RT1(0);
+            rk_tau = kRkB5[TAB][0] * RT1(3);
+            rk_I = kRkB5[TAB][0] * RT1(4) * d_exp_lo(-tau_n);
+            K.set(4, 0, RT1(3));
+        }
         // The stage argument (ir, ith, ipr, ipth), the slope k and sinθ, cosθ are declared OUTSIDE the stage
         // loop: after its last trip they hold the end state and f(end state), so no second set of
         // loop-carried registers (and no copies at the loop head) is needed for them.
@@ -177,6 +190,23 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             }
             if (ev) {
                 geodesic_rhs(a, a2, L, ir, ith, ipr, ipth, k, sn, cn);
+                if (RTS == 1 && s < 6) {                                   // coefficients at this stage state
+                    RtPoint pt; rt_point<false>(P, L, ir, sn, cn, ipr, pt);
+                    double as, es; rt_coefficients<false>(P, pt, 0, as, es);
+                    double ts = 0.0;
+                    switch (s) {
+                        case 1: ts = stage_sum<TAB, 1>(K, 4); break;
+                        case 2: ts = stage_sum<TAB, 2>(K, 4); break;
+                        case 3: ts = stage_sum<TAB, 3>(K, 4); break;
+                        case 4: ts = stage_sum<TAB, 4>(K, 4); break;
+                        default: ts = stage_sum<TAB, 5>(K, 4); break;
+                    }
+                    const double b5s = (s == 1) ? kRkB5[TAB][1] : (s == 2) ? kRkB5[TAB][2] : (s == 3) ? kRkB5[TAB][3]
+                                     : (s == 4) ? kRkB5[TAB][4] : kRkB5[TAB][5];
+                    rk_tau = fma(b5s, as, rk_tau);
+                    rk_I = fma(b5s * es, d_exp_lo(-fma(h_try, ts, tau_n)), rk_I);
+                    K.set(4, s, as);
+                }
                 switch (s) {
                     case 1: store_stage<TAB, 1>(K, k, ph5, phe); break;
                     case 2: store_stage<TAB, 2>(K, k, ph5, phe); break;
@@ -231,7 +261,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
 
         // ------------------------------------------------------------------ radiative transfer over the step taken
         if (KIND == 2 && (commit || fresh)) {
-            RtPoint pt; rt_point(P, L, yn.r, sn, cn, yn.pr, pt);
+            RtPoint pt; rt_point<SPEC>(P, L, yn.r, sn, cn, yn.pr, pt);
             bool all_opaque = true;
             if (SPEC) {
 #pragma unroll 4
@@ -240,15 +270,23 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     // unrolled iterations are independent chains the scheduler can interleave
                     double tk = ACC(0, k), Tk = ACC(1, k), Ik = ACC(2, k);
                     const double a0k = ACC(3, k), e0k = ACC(4, k);
-                    double a1, e1; rt_coefficients(P, pt, k, a1, e1);
+                    double a1, e1; rt_coefficients<true>(P, pt, k, a1, e1);
                     rt_update(a0k, a1, e0k, e1, commit ? h_try : 0.0, P.tau_max, tk, Tk, Ik);   // fresh lane: zero-length step
                     ACC(0, k) = tk; ACC(1, k) = Tk; ACC(2, k) = Ik;
                     if (!(tk > P.tau_max)) all_opaque = false;
                     ACC(3, k) = a1; ACC(4, k) = e1;
                 }
             } else {
-                double a1, e1; rt_coefficients(P, pt, 0, a1, e1);
-                if (commit) {
+                double a1, e1; rt_coefficients<false>(P, pt, 0, a1, e1);
+                if (commit && RTS == 1) {
+                    double tau = RT1(0);
+                    if (!(tau > P.tau_max)) {                              // frozen once tau > tau_max
+                        RT1(2) = fma(h_try, rk_I, RT1(2));
+                        tau = fma(h_try, rk_tau, tau);
+                        RT1(0) = tau;
+                    }
+                    all_opaque = (tau > P.tau_max);
+                } else if (commit) {
                     double tau = RT1(0), Tr = RT1(1), Inu = RT1(2);
                     rt_update(RT1(3), a1, RT1(4), e1, h_try, P.tau_max, tau, Tr, Inu);
                     RT1(0) = tau; RT1(1) = Tr; RT1(2) = Inu;

@@ -37,7 +37,7 @@ struct Params {
     double inv_planck;                          // c²/(2h)
     double r_rt_out, tau_max, rg_cm;
     double sed_coef;                            // 4π r_g^2 Δx Δy
-    int32_t nf, pad;
+    int32_t nf, rt_scheme;                      // rt_scheme: ODYSSEY_RT_* (kind 2)
     double nu[MAX_FREQ];
     double ln_nu[MAX_FREQ];
     double nu12[MAX_FREQ], inu12[MAX_FREQ];     // ν^(1/12) and its reciprocal (eq. (38) in powers of x_M^(1/12))

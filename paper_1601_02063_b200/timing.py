@@ -55,6 +55,7 @@ def main():
     import torch
     import paper_1601_02063_b200 as ody
     cases = [("C0", W.C0()), ("C1", W.C1()), ("C2", W.C2()), ("C3", W.C3()), ("C4", W.C4())]
+    cases.append(("C2 rt_scheme=RK components", dict(W.C2(), model=W.model_riaf(rt_scheme=W.RT_RK_COMPONENTS))))
     if args.sweep:
         for a in (0.0, 0.5, 0.9, 0.998):
             for n in (1024, 2048, 4096):

@@ -32,7 +32,7 @@ def test_header_symbols_are_all_exported():
 def test_struct_layout_matches_header_sizes():
     # 8 doubles + 2 int32 + double + 2 int32 + 3 doubles + 2 int32 = 15*8 = 120 bytes; model: 2 int32 + 16 doubles
     assert C.sizeof(B.Scene) == 120
-    assert C.sizeof(B.Model) == 8 + 16 * 8
+    assert C.sizeof(B.Model) == 8 + 16 * 8 + 8
 
 
 @pytest.mark.parametrize("patch, msg", [
@@ -58,6 +58,12 @@ def test_invalid_model_and_frequencies_are_rejected():
     assert L.odyssey_render_spectrum(C.byref(sc), C.byref(mo), nu, 8, None, None, None, None, None) == -1
     bad = dict(w["model"]); bad["kind"] = 9
     assert L.odyssey_render_image(C.byref(sc), C.byref(B._struct(B.Model, bad)), C.c_double(1e9),
+                                  None, None, None, None, None, None, None, None) == -1
+    rk = B._struct(B.Model, dict(w["model"], rt_scheme=W.RT_RK_COMPONENTS))
+    assert L.odyssey_render_spectrum(C.byref(sc), C.byref(rk), nu, 4, None, None, None, None, None) == -1
+    assert "rt_scheme" in ody.last_error()
+    bad_rt = B._struct(B.Model, dict(w["model"], rt_scheme=5))
+    assert L.odyssey_render_image(C.byref(sc), C.byref(bad_rt), C.c_double(1e9),
                                   None, None, None, None, None, None, None, None) == -1
     thin = B._struct(B.Model, W.C1()["model"])
     assert L.odyssey_render_spectrum(C.byref(sc), C.byref(thin), nu, 4, None, None, None, None, None) == -1

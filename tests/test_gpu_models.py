@@ -165,3 +165,24 @@ def test_c4_full_size_sampled(ody, orc):
     n_att = _np(out["n_attempt"])
     assert n_att.min() > 0 and n_att.max() < w["scene"]["max_attempts"]
     assert np.mean(_sub(n_att, idx) == ref["n_attempt"]) >= 0.995
+
+
+# ------------------------------------------------------------------------- transfer scheme E' (RK components)
+@pytest.mark.parametrize("nu, tableau", [(230.0e9, W.TABLEAU_RKF45), (30.0e9, W.TABLEAU_RKF45), (230.0e9, W.TABLEAU_CASH_KARP)])
+def test_rk_component_transfer_scheme_matches_the_oracle(ody, orc, nu, tableau):
+    w = W.C2(n=64)
+    sc = dict(w["scene"], tableau=tableau)
+    mo = dict(w["model"], rt_scheme=W.RT_RK_COMPONENTS)
+    out = ody.render_image(sc, mo, nu); _sync()
+    ref = orc.render_image(sc, mo, nu)
+    assert np.array_equal(_np(out["flag"]).ravel(), ref["flag"])
+    _check_image(_np(out["image"]).ravel(), ref["image"], f"RK-component scheme at {nu:g} Hz")
+    tau, tr = _np(out["aux0"]).ravel(), ref["aux0"]
+    assert np.max(np.abs(tau - tr) / np.maximum(tr, 1e-6 * tr.max())) <= 1e-4
+    # same geodesics, same steps as the default scheme
+    base = ody.render_image(sc, w["model"], nu); _sync()
+    opaque = (ref["flag"] == W.FLAG_OPAQUE) | (_np(base["flag"]).ravel() == W.FLAG_OPAQUE)
+    assert np.array_equal(_np(out["n_attempt"]).ravel()[~opaque], _np(base["n_attempt"]).ravel()[~opaque])
+    # and the two discretisations agree to their truncation error
+    a, b = _np(out["image"]).ravel(), _np(base["image"]).ravel()
+    assert np.abs(a - b).sum() / b.sum() < 5e-3
