@@ -54,6 +54,13 @@ int device_state(DevState** out, int* dev_out) {
             return fail(ODYSSEY_ERR_UNSUPPORTED_DEVICE, "device %d is sm_%d%d; this library is built for sm_100a only", dev, prop.major, prop.minor);
         D.n_sm = prop.multiProcessorCount;
         CUDA_TRY(cudaMalloc(&D.ring, RING * sizeof(unsigned long long)));
+        // stream-ordered scratch (spectrum accumulators, the _host variants' device buffers) comes from the
+        // device's default pool; keep freed blocks cached instead of returning them at every synchronisation
+        cudaMemPool_t pool = nullptr;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
         D.ready = true;
     }
     *out = &D; if (dev_out) *dev_out = dev;
@@ -219,12 +226,12 @@ Outputs no_outputs() { Outputs O; std::memset(&O, 0, sizeof(O)); return O; }
 namespace {
 struct Scratch {
     void* dev[12]; void* host[12]; size_t bytes[12]; int n = 0;
-    ~Scratch() { for (int i = 0; i < n; ++i) if (dev[i]) cudaFree(dev[i]); }
+    ~Scratch() { for (int i = 0; i < n; ++i) if (dev[i]) cudaFreeAsync(dev[i], 0); }
     template <class T> int add(T* host_ptr, size_t count, T** out) {
         *out = nullptr;
         if (!host_ptr) return ODYSSEY_OK;
         void* d = nullptr;
-        CUDA_TRY(cudaMalloc(&d, count * sizeof(T)));
+        CUDA_TRY(cudaMallocAsync(&d, count * sizeof(T), 0));
         dev[n] = d; host[n] = host_ptr; bytes[n] = count * sizeof(T); ++n;
         *out = (T*)d;
         return ODYSSEY_OK;
@@ -383,6 +390,8 @@ void odyssey_shutdown(void) {
         if (!g_dev[d].ready) continue;
         cudaSetDevice(d);
         cudaFree(g_dev[d].ring);
+        cudaMemPool_t pool = nullptr;
+        if (cudaDeviceGetDefaultMemPool(&pool, d) == cudaSuccess) { cudaDeviceSynchronize(); cudaMemPoolTrimTo(pool, 0); }
         g_dev[d] = DevState();
     }
     cudaSetDevice(cur);
