@@ -1,0 +1,42 @@
+"""Writes tests/golden/oracle_regression.json from the CPU oracle ALONE (never from the CUDA path): a few
+oracle outputs on tiny grids, so that an accidental change to the oracle's arithmetic shows up as a diff.
+A deliberate change re-runs this script and names, in its commit message, the PAPER.md passage or
+DESIGN.md reading that justifies it.
+
+    python tests/golden/make_oracle_golden.py
+"""
+import json
+import os
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, os.path.dirname(os.path.dirname(HERE)))
+
+import workloads as W  # noqa: E402
+from oracle import binding as O  # noqa: E402
+
+
+def main():
+    out = {"_comment": "written by tests/golden/make_oracle_golden.py from oracle/ only"}
+    w = W.C0(n=8)
+    g = O.trace_geodesics(w["scene"])
+    out["C0_8x8"] = {k: g[k].tolist() for k in ("flag", "r", "th", "ph", "n_attempt", "n_accept")}
+    w = W.C1(n=8)
+    d = O.render_image(w["scene"], w["model"])
+    out["C1_8x8"] = {"flag": d["flag"].tolist(), "g": d["aux0"].tolist(), "r_e": d["aux1"].tolist(),
+                     "image": d["image"].tolist()}
+    w = W.C2(n=8)
+    for scheme in (W.RT_PER_STEP, W.RT_RK_COMPONENTS):
+        r = O.render_image(w["scene"], dict(w["model"], rt_scheme=scheme), w["nu"][0])
+        out[f"C2_8x8_rt_scheme{scheme}"] = {"flag": r["flag"].tolist(), "image": r["image"].tolist(),
+                                            "tau": r["aux0"].tolist(), "n_attempt": r["n_attempt"].tolist()}
+    w = W.C3(n=4, nf=4)
+    s = O.render_spectrum(w["scene"], w["model"], w["nu"])
+    out["C3_4x4_nf4"] = {"nu": list(w["nu"]), "nuLnu": s["nuLnu"].tolist(), "images": s["images"].tolist()}
+    with open(os.path.join(HERE, "oracle_regression.json"), "w") as f:
+        json.dump(out, f, indent=1)
+    print("wrote oracle_regression.json")
+
+
+if __name__ == "__main__":
+    main()
