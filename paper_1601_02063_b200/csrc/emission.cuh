@@ -138,13 +138,19 @@ __device__ __forceinline__ void rt_point(const Params& P, const double L, const 
 }
 
 // Per-frequency coefficients.  ln_nu = ln ν_k.
+// Per-frequency constants.  The fused kernels index the Params tables with a warp-uniform k (uniform
+// constant loads); the two-phase spectrum kernel, where k is the LANE's frequency, must fetch them once into
+// registers — a constant load with 32 different addresses is replayed 32 times.
+struct Freq { double nu, ln_nu, nu12, inu12; };
+__device__ __forceinline__ Freq freq_of(const Params& P, const int k) { return Freq{P.nu[k], P.ln_nu[k], P.nu12[k], P.inu12[k]}; }
+
 template <bool HOIST>
-__device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& q, const int k, double& acoef, double& ecoef) {
-    const double nu = P.nu[k], ln_nu = P.ln_nu[k];
+__device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& q, const Freq& f, double& acoef, double& ecoef) {
+    const double nu = f.nu, ln_nu = f.ln_nu;
     // straight-line on purpose (no early return when the point is off: fac = 0 gives ε = a = 0), so that the
     // spectrum kernel's unrolled frequency loop can interleave independent chains
     double t, u;                                                     // x_M^(1/12) and its reciprocal
-    if (HOIST) { t = q.t0 * P.nu12[k]; u = q.u0 * P.inu12[k]; }
+    if (HOIST) { t = q.t0 * f.nu12; u = q.u0 * f.inu12; }
     else { t = d_exp_nc((ln_nu + q.lxm0) * (1.0 / 12.0)); u = d_rcp(t); }
     const double t2 = t * t, u2 = u * u;
     const double u3 = u2 * u;

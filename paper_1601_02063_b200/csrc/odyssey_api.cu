@@ -31,6 +31,7 @@ int fail(int code, const char* fmt, ...) {
     return code;
 }
 
+#define TRY_RC(expr) do { int rc_ = (expr); if (rc_) return rc_; } while (0)
 #define CUDA_TRY(expr)                                                                             \
     do { cudaError_t e_ = (expr);                                                                  \
          if (e_ != cudaSuccess) return fail(ODYSSEY_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
@@ -169,6 +170,8 @@ typedef void (*KernelFn)(const Params, const Outputs);
 KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0) {
     if (kind == 2 && !spec && rts == 1)
         return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_RK, 1> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_RK, 1>;
+    if (kind == 2 && !spec && rts == 2)
+        return tab ? odyssey_kernel<2, 1, false, NT_MAIN, 4, 2> : odyssey_kernel<2, 0, false, NT_MAIN, 4, 2>;
     if (spec) return tab ? odyssey_kernel<2, 1, true, NT_SPEC, MINB_SPEC> : odyssey_kernel<2, 0, true, NT_SPEC, MINB_SPEC>;
     switch (kind) {
         case 0: return tab ? odyssey_kernel<0, 1, false, NT_MAIN, MINB_MAIN> : odyssey_kernel<0, 0, false, NT_MAIN, MINB_MAIN>;
@@ -219,6 +222,77 @@ int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
 }
 
 Outputs no_outputs() { Outputs O; std::memset(&O, 0, sizeof(O)); return O; }
+
+// ---- two-phase spectrum path (small images; see spectrum_rt_kernel in odyssey_kernels.cuh) ------------------
+// Used when the image has fewer rays than TWO_PHASE_WAVES waves of resident lanes: there the fused spectrum
+// kernel's run time is the serial time of the longest ray.  Phases: count pass (record kernel without a node
+// buffer: its n_accept sizes the node lists), prefix sum, ONE stream synchronisation to read the node total,
+// record pass, per-frequency transfer with one lane per (ray, frequency).
+constexpr int TWO_PHASE_WAVES = 4;
+
+template <int G>
+cudaError_t launch_spectrum_rt(const Params& P, const Outputs& O, int blocks, cudaStream_t st) {
+    spectrum_rt_kernel<G><<<blocks, 128, 0, st>>>(P, O);
+    return cudaGetLastError();
+}
+
+int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st) {
+    DevState* D = nullptr;
+    TRY_RC(device_state(&D, nullptr));
+    const size_t n = (size_t)P.nx * P.ny;
+    int32_t *iflag = nullptr, *iatt = nullptr, *iacc = nullptr; long long* off = nullptr; double* nodes = nullptr;
+    auto release = [&]() {
+        if (iflag) cudaFreeAsync(iflag, st); if (iatt) cudaFreeAsync(iatt, st); if (iacc) cudaFreeAsync(iacc, st);
+        if (off) cudaFreeAsync(off, st); if (nodes) cudaFreeAsync(nodes, st);
+    };
+#define TP_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { release(); return fail(ODYSSEY_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } } while (0)
+    TP_TRY(cudaMallocAsync((void**)&iflag, n * sizeof(int32_t), st));
+    TP_TRY(cudaMallocAsync((void**)&iatt, n * sizeof(int32_t), st));
+    TP_TRY(cudaMallocAsync((void**)&iacc, n * sizeof(int32_t), st));
+    TP_TRY(cudaMallocAsync((void**)&off, (n + 1) * sizeof(long long), st));
+    Params Pr = P; Pr.rt_scheme = 2; Pr.nf = 1;
+    Outputs O1 = no_outputs();
+    O1.flag = iflag; O1.n_attempt = iatt; O1.n_accept = iacc;
+    int rc = launch(Pr, O1, false, tab, st);                                   // count pass
+    if (rc) { release(); return rc; }
+    node_offsets_kernel<<<1, 1024, 0, st>>>(iacc, (int)n, off);
+    TP_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+    long long total = 0;
+    TP_TRY(cudaMemcpyAsync(&total, off + n, sizeof(long long), cudaMemcpyDeviceToHost, st));
+    TP_TRY(cudaStreamSynchronize(st));
+    TP_TRY(cudaMallocAsync((void**)&nodes, (size_t)total * NODE_DOUBLES * sizeof(double), st));
+    O1.nodes = nodes; O1.node_offset = off;
+    rc = launch(Pr, O1, false, tab, st);                                       // record pass
+    if (rc) { release(); return rc; }
+    Outputs O2 = no_outputs();
+    O2.images = user.images; O2.nuLnu = user.nuLnu; O2.flag = user.flag; O2.n_attempt = user.n_attempt;
+    O2.nodes = nodes; O2.node_offset = off;
+    O2.queue = next_counter(D);
+    TP_TRY(cudaMemsetAsync(O2.queue, 0, sizeof(unsigned long long), st));
+    if (user.nuLnu) TP_TRY(cudaMemsetAsync(user.nuLnu, 0, sizeof(double) * P.nf, st));
+    if (user.flag) TP_TRY(cudaMemcpyAsync(user.flag, iflag, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    if (user.n_attempt) TP_TRY(cudaMemcpyAsync(user.n_attempt, iatt, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    O2.aux_flag = iflag;
+    int G = 1; while (G < P.nf) G <<= 1;
+    const long long warps = ((long long)n + 32 / G - 1) / (32 / G);
+    long long blocks = std::min<long long>((warps + 3) / 4, (long long)D->n_sm * 16);
+    if (blocks < 1) blocks = 1;
+    cudaError_t le = cudaSuccess;
+    switch (G) {
+        case 1: le = launch_spectrum_rt<1>(P, O2, (int)blocks, st); break;
+        case 2: le = launch_spectrum_rt<2>(P, O2, (int)blocks, st); break;
+        case 4: le = launch_spectrum_rt<4>(P, O2, (int)blocks, st); break;
+        case 8: le = launch_spectrum_rt<8>(P, O2, (int)blocks, st); break;
+        case 16: le = launch_spectrum_rt<16>(P, O2, (int)blocks, st); break;
+        default: le = launch_spectrum_rt<32>(P, O2, (int)blocks, st); break;
+    }
+    TP_TRY(le);
+    g_launches.fetch_add(1);
+#undef TP_TRY
+    release();
+    return ODYSSEY_OK;
+}
 
 }  // namespace
 
@@ -290,6 +364,12 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
     Params P; fill_params(*scene, model, nu_hz_host, nf, &P);
     Outputs O = no_outputs();
     O.images = images; O.nuLnu = nuLnu; O.flag = flag; O.n_attempt = n_attempt;
+    DevState* D = nullptr;
+    rc = device_state(&D, nullptr);
+    if (rc) return rc;
+    const long long lanes = (long long)D->n_sm * 4 * NT_MAIN;                  // resident lanes of the record kernel
+    if ((long long)scene->nx * scene->ny <= TWO_PHASE_WAVES * lanes)
+        return render_spectrum_two_phase(P, O, scene->tableau, (cudaStream_t)cuda_stream);
     return launch(P, O, true, scene->tableau, (cudaStream_t)cuda_stream);
 }
 

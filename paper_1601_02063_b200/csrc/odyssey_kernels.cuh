@@ -56,9 +56,10 @@ __device__ __forceinline__ void store_stage(KS& K, const Slope& k, double& ph5, 
 
 // Shared-memory doubles per thread: rows x 6 stage values + 5 single-frequency transfer values
 // (rows = 4 slopes, + the absorption coefficient for transfer scheme E').
-__host__ __device__ constexpr int smem_per_thread(int rts) { return (rts ? STAGE_ROWS : STAGE_ROWS - 1) * 6 + 5; }
+__host__ __device__ constexpr int smem_per_thread(int rts) { return (rts == 1 ? STAGE_ROWS : STAGE_ROWS - 1) * 6 + 5; }
 
 // RTS = 1: transfer scheme E' (tau, I as Runge–Kutta components; single frequency only).
+// RTS = 2: record mode, the first phase of the two-phase spectrum path (see spectrum_rt_kernel below).
 template <int KIND, int TAB, bool SPEC, int NT, int MINB, int RTS = 0>
 __global__ void __launch_bounds__(NT, MINB)
 odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs O) {
@@ -192,7 +193,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                 geodesic_rhs(a, a2, L, ir, ith, ipr, ipth, k, sn, cn);
                 if (RTS == 1 && s < 6) {                                   // coefficients at this stage state
                     RtPoint pt; rt_point<false>(P, L, ir, sn, cn, ipr, pt);
-                    double as, es; rt_coefficients<false>(P, pt, 0, as, es);
+                    double as, es; rt_coefficients<false>(P, pt, freq_of(P, 0), as, es);
                     double ts = 0.0;
                     switch (s) {
                         case 1: ts = stage_sum<TAB, 1>(K, 4); break;
@@ -260,7 +261,18 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         }
 
         // ------------------------------------------------------------------ radiative transfer over the step taken
-        if (KIND == 2 && (commit || fresh)) {
+        if (KIND == 2 && RTS == 2) {
+            // RECORD mode (first phase of the two-phase spectrum path): no transfer here; the per-point
+            // quantities all frequencies share go to the ray's node list (node 0 = start point, node j = end of
+            // accepted step j).  With O.nodes == nullptr this is the COUNT pass: same code, same steps,
+            // nothing written (its n_accept sizes the node lists).  The ray never ends OPAQUE here.
+            if ((commit || fresh) && O.nodes) {
+                RtPoint pt; rt_point<true>(P, L, yn.r, sn, cn, yn.pr, pt);
+                double* nd = O.nodes + NODE_DOUBLES * (O.node_offset[pix] + (long long)(fresh ? 0 : n_acc));
+                nd[0] = fresh ? 0.0 : h_try; nd[1] = pt.fac; nd[2] = pt.E; nd[3] = pt.t0; nd[4] = pt.u0; nd[5] = pt.ycoef;
+                nd[6] = (double)n_att;
+            }
+        } else if (KIND == 2 && (commit || fresh)) {
             RtPoint pt; rt_point<SPEC>(P, L, yn.r, sn, cn, yn.pr, pt);
             bool all_opaque = true;
             if (SPEC) {
@@ -270,14 +282,14 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     // unrolled iterations are independent chains the scheduler can interleave
                     double tk = ACC(0, k), Tk = ACC(1, k), Ik = ACC(2, k);
                     const double a0k = ACC(3, k), e0k = ACC(4, k);
-                    double a1, e1; rt_coefficients<true>(P, pt, k, a1, e1);
+                    double a1, e1; rt_coefficients<true>(P, pt, freq_of(P, k), a1, e1);
                     rt_update(a0k, a1, e0k, e1, commit ? h_try : 0.0, P.tau_max, tk, Tk, Ik);   // fresh lane: zero-length step
                     ACC(0, k) = tk; ACC(1, k) = Tk; ACC(2, k) = Ik;
                     if (!(tk > P.tau_max)) all_opaque = false;
                     ACC(3, k) = a1; ACC(4, k) = e1;
                 }
             } else {
-                double a1, e1; rt_coefficients<false>(P, pt, 0, a1, e1);
+                double a1, e1; rt_coefficients<false>(P, pt, freq_of(P, 0), a1, e1);
                 if (commit && RTS == 1) {
                     double tau = RT1(0);
                     if (!(tau > P.tau_max)) {                              // frozen once tau > tau_max
@@ -325,6 +337,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     if (b >= P.nbins) b = P.nbins - 1;
                     atomicAdd(&sm_red[b], val * P.pix_area);
                 }
+            } else if (RTS == 2) {
+                // record mode: flag and step counts only (written above)
             } else if (!SPEC) {
                 if (O.image) O.image[pix] = P.nu3[0] * RT1(2);
                 if (O.aux0) O.aux0[pix] = RT1(0);
@@ -351,6 +365,110 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         __syncthreads();
         for (int k = threadIdx.x; k < P.nbins; k += NT) if (sm_red[k] != 0.0) atomicAdd(&O.hist[k], sm_red[k]);
     }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Two-phase spectrum path for small images (fewer rays than a few waves of lanes).  With one ray per
+// lane and nothing left in the queue, the fused spectrum kernel's run time is the serial time of the
+// longest ray with all nf frequencies behind each other.  Here phase 1 (odyssey_kernel<2, TAB, false, …,
+// RTS = 2>) integrates the geodesics once and records one node per accepted step; phase 2 below gives
+// every ray a group of G >= nf lanes, one frequency per lane, and walks the node list: the transfer of
+// the nf frequencies runs side by side, and rays are handed out through an atomic counter.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) node_offsets_kernel(const int32_t* __restrict__ n_accept, int n,
+                                                             long long* __restrict__ offset /* [n + 1] */) {
+    __shared__ long long part[1024];
+    const int t = threadIdx.x;
+    const int per = (n + 1023) / 1024, lo = min(t * per, n), hi = min(lo + per, n);
+    long long s = 0;
+    for (int i = lo; i < hi; ++i) s += n_accept[i] + 1;                 // nodes of ray i: start point + accepted steps
+    part[t] = s;
+    __syncthreads();
+    for (int d = 1; d < 1024; d <<= 1) {                                 // inclusive Hillis–Steele scan
+        const long long v = (t >= d) ? part[t - d] : 0;
+        __syncthreads();
+        part[t] += v;
+        __syncthreads();
+    }
+    long long run = part[t] - s;                                         // exclusive prefix of this thread's chunk
+    for (int i = lo; i < hi; ++i) { offset[i] = run; run += n_accept[i] + 1; }
+    if (t == 1023) offset[n] = part[1023];
+}
+
+template <int G>                                                         // lanes per ray: power of two, nf <= G <= 32
+__global__ void __launch_bounds__(128, 5) spectrum_rt_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs O) {
+    __shared__ double sed[MAX_FREQ];
+    for (int k = threadIdx.x; k < MAX_FREQ; k += blockDim.x) sed[k] = 0.0;
+    __syncthreads();
+    constexpr int RPW = 32 / G;                                          // rays per warp
+    const int lane = threadIdx.x & 31, k = lane % G, sub = lane / G;
+    const unsigned gmask = (G == 32) ? FULL : (((1u << G) - 1u) << (sub * G));
+    const int nf = P.nf, npix = P.nx * P.ny;
+    const bool fk = k < nf;                                              // this lane owns a frequency
+    Freq fq = freq_of(P, fk ? k : 0);                                    // lane-constant: fetched once (divergent constant loads)
+    double nu3 = P.nu3[fk ? k : 0];
+    // pin the values in registers: without this the compiler re-materialises them with a constant load at every use
+    asm volatile("" : "+d"(fq.nu), "+d"(fq.ln_nu), "+d"(fq.nu12), "+d"(fq.inu12), "+d"(nu3));
+    for (;;) {
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(O.queue, (unsigned long long)RPW);
+        base = __shfl_sync(FULL, base, 0);
+        if (base >= (unsigned long long)npix) break;
+        const int pix = (int)base + sub;
+        const bool live = pix < npix;
+        const long long off = live ? O.node_offset[pix] : 0;
+        const int cnt = live ? (int)(O.node_offset[pix + 1] - off) : 0;
+        // a step that ended the ray by capture or escape keeps that flag even if it also made the ray opaque
+        // (the fused kernel tests the events before the transfer update); a MAXSTEP ray's last step may end OPAQUE
+        const int end_flag = live ? O.aux_flag[pix] : F_MAXSTEP;
+        const int last_opaque_ok = (end_flag == F_CAPTURED || end_flag == F_ESCAPED) ? cnt - 1 : cnt;
+        int cmax = cnt;
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) cmax = max(cmax, __shfl_xor_sync(FULL, cmax, d));
+        // Software pipeline: the coefficients of node i+1 (two exponentials, independent of everything before)
+        // are evaluated in the same trip as the update over step i (a serial recurrence in tau, T, I), and
+        // node i+2 is already being loaded — three independent chains per lane.
+        double tau = 0.0, T = 1.0, I = 0.0;
+        bool done = !live;
+        int opaque_att = -1;
+        auto load_node = [&](int i, RtPoint& pt, double& h, double& natt) {
+            pt.on = true;
+            if (i < cnt) {
+                const double* nd = O.nodes + NODE_DOUBLES * (off + i);
+                h = __ldg(nd); pt.fac = __ldg(nd + 1); pt.E = __ldg(nd + 2); pt.t0 = __ldg(nd + 3); pt.u0 = __ldg(nd + 4);
+                pt.ycoef = __ldg(nd + 5); natt = __ldg(nd + 6);
+            } else { h = 0.0; natt = 0.0; pt.fac = 0.0; pt.E = 0.0; pt.t0 = 1.0; pt.u0 = 1.0; pt.ycoef = 0.0; }
+        };
+        RtPoint p0, p1, p2; double h0, h1, h2, n0, n1, n2;
+        load_node(0, p0, h0, n0); load_node(1, p1, h1, n1); load_node(2, p2, h2, n2);
+        double a_prev, e_prev, a_cur, e_cur;
+        rt_coefficients<true>(P, p0, fq, a_prev, e_prev);                // node 0: start point
+        rt_coefficients<true>(P, p1, fq, a_cur, e_cur);                  // node 1
+        for (int i = 1; i < cmax; ++i) {
+            RtPoint p3; double h3, n3;
+            load_node(i + 2, p3, h3, n3);                                // two ahead
+            double a_nxt, e_nxt;
+            rt_coefficients<true>(P, p2, fq, a_nxt, e_nxt);              // node i+1
+            const bool step = !done && i < cnt;
+            if (step) rt_update(a_prev, a_cur, e_prev, e_cur, h1, P.tau_max, tau, T, I);   // step i (ends at node i)
+            // the ray is opaque once every one of its frequencies is (lanes without a frequency vote yes)
+            const unsigned votes = __ballot_sync(FULL, !fk || (tau > P.tau_max));
+            if (step && i < last_opaque_ok && (votes & gmask) == gmask) { done = true; opaque_att = (int)n1; }
+            a_prev = a_cur; e_prev = e_cur; a_cur = a_nxt; e_cur = e_nxt;
+            h1 = h2; n1 = n2; p2 = p3; h2 = h3; n2 = n3;
+        }
+        if (live && fk) {
+            const double v = nu3 * I;
+            if (O.images) O.images[(size_t)k * npix + pix] = v;
+            if (O.nuLnu) atomicAdd(&sed[k], v);
+        }
+        if (live && k == 0 && opaque_att >= 0) {                         // the fused kernel's OPAQUE ending
+            if (O.flag) O.flag[pix] = F_OPAQUE;
+            if (O.n_attempt) O.n_attempt[pix] = opaque_att;
+        }
+    }
+    __syncthreads();
+    if (O.nuLnu) for (int q = threadIdx.x; q < nf; q += blockDim.x) if (sed[q] != 0.0) atomicAdd(&O.nuLnu[q], P.sed_coef * P.nu[q] * sed[q]);
 }
 
 // Diagnostic kernel behind odyssey_eval_math: the device elementary functions, elementwise.

@@ -9,6 +9,7 @@ namespace ody {
 constexpr int MAX_FREQ = 32;
 constexpr int TILE_W = 8, TILE_H = 4;          // one queue tile = 8x4 pixels = one warp's first batch
 constexpr int LOCATE_MAX = 8;                  // Newton re-attempts of the event location
+constexpr int NODE_DOUBLES = 7;                // two-phase spectrum path: h, fac, E, t0, u0, ycoef, n_attempt per node
 
 struct Params {
     // ---- scene
@@ -53,6 +54,9 @@ struct Outputs {
     double* hist;                                // kind 1
     double* images; double* nuLnu;               // spectrum mode
     double* spec_state;                          // spectrum mode: library scratch, [5][nf][grid threads] accumulators
+    double* nodes;                               // two-phase spectrum path: library scratch, NODE_DOUBLES per node
+    const long long* node_offset;                // two-phase spectrum path: first node of each ray, [npix + 1]
+    const int32_t* aux_flag;                     // two-phase spectrum path: the record pass's flags (input of phase 2)
     unsigned long long* queue;                   // work-queue counter (zeroed before the launch)
 };
 
