@@ -119,7 +119,10 @@ int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model,
 
 /* nf <= 32 observed frequencies integrated simultaneously along each geodesic (kind 2 only;
  * BASELINE.json:configs[3]).  images[nf][ny][nx] = I_nu; nuLnu[nf] = 4π nu r_g^2 Δx Δy Σ_pixels I_nu
- * (erg/s; the distance cancels).  nu_hz_host is HOST memory.                                      */
+ * (erg/s; the distance cancels).  nu_hz_host is HOST memory.  rt_scheme must be ODYSSEY_RT_PER_STEP.
+ * Images with fewer rays than four waves of resident lanes (~3e5 pixels on a B200) take a two-phase path
+ * (record the geodesics once, then one lane per (ray, frequency)); that path synchronises `cuda_stream`
+ * ONCE inside the call to read an overflow flag, and uses stream-ordered scratch (up to 28 KB per ray).   */
 int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* model,
                             const double* nu_hz_host, int nf,
                             double* images, double* nuLnu, int32_t* flag, int32_t* n_attempt,

@@ -225,10 +225,11 @@ Outputs no_outputs() { Outputs O; std::memset(&O, 0, sizeof(O)); return O; }
 
 // ---- two-phase spectrum path (small images; see spectrum_rt_kernel in odyssey_kernels.cuh) ------------------
 // Used when the image has fewer rays than TWO_PHASE_WAVES waves of resident lanes: there the fused spectrum
-// kernel's run time is the serial time of the longest ray.  Phases: count pass (record kernel without a node
-// buffer: its n_accept sizes the node lists), prefix sum, ONE stream synchronisation to read the node total,
-// record pass, per-frequency transfer with one lane per (ray, frequency).
+// kernel's run time is the serial time of the longest ray.  Phases: record pass into fixed-capacity node lists,
+// ONE stream synchronisation to read its overflow flag (on overflow: count pass, prefix sum, exact-size record
+// pass), then the per-frequency transfer with one lane per (ray, frequency).
 constexpr int TWO_PHASE_WAVES = 4;
+constexpr long long NODE_CAP = 512;            // nodes per ray of the first, fixed-capacity attempt (28 KB per ray)
 
 template <int G>
 cudaError_t launch_spectrum_rt(const Params& P, const Outputs& O, int blocks, cudaStream_t st) {
@@ -253,21 +254,44 @@ int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st) 
     Params Pr = P; Pr.rt_scheme = 2; Pr.nf = 1;
     Outputs O1 = no_outputs();
     O1.flag = iflag; O1.n_attempt = iatt; O1.n_accept = iacc;
-    int rc = launch(Pr, O1, false, tab, st);                                   // count pass
+    // First try: ONE record pass into fixed-capacity node lists (NODE_CAP nodes per ray) and an overflow flag.
+    int32_t* ovf = nullptr;
+    TP_TRY(cudaMallocAsync((void**)&ovf, sizeof(int32_t), st));
+    TP_TRY(cudaMemsetAsync(ovf, 0, sizeof(int32_t), st));
+    TP_TRY(cudaMallocAsync((void**)&nodes, n * NODE_CAP * NODE_DOUBLES * sizeof(double), st));
+    O1.nodes = nodes; O1.node_cap = NODE_CAP; O1.overflow = ovf;
+    int rc = launch(Pr, O1, false, tab, st);
+    int32_t overflow = 0;
+    if (rc == ODYSSEY_OK) {
+        cudaError_t e1 = cudaMemcpyAsync(&overflow, ovf, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(st);                 // the one synchronisation of this path
+        if (e1 != cudaSuccess) rc = fail(ODYSSEY_ERR_CUDA, "two-phase spectrum: %s", cudaGetErrorString(e1));
+    }
+    cudaFreeAsync(ovf, st);
     if (rc) { release(); return rc; }
-    node_offsets_kernel<<<1, 1024, 0, st>>>(iacc, (int)n, off);
-    TP_TRY(cudaGetLastError());
-    g_launches.fetch_add(1);
-    long long total = 0;
-    TP_TRY(cudaMemcpyAsync(&total, off + n, sizeof(long long), cudaMemcpyDeviceToHost, st));
-    TP_TRY(cudaStreamSynchronize(st));
-    TP_TRY(cudaMallocAsync((void**)&nodes, (size_t)total * NODE_DOUBLES * sizeof(double), st));
-    O1.nodes = nodes; O1.node_offset = off;
-    rc = launch(Pr, O1, false, tab, st);                                       // record pass
-    if (rc) { release(); return rc; }
+    long long node_cap = NODE_CAP;
+    if (overflow) {
+        // Some ray took more accepted steps than NODE_CAP - 1 (tight tolerances): size the lists exactly —
+        // count pass (same kernel, no node buffer), prefix sum, read the total, record again.
+        cudaFreeAsync(nodes, st); nodes = nullptr;
+        O1.nodes = nullptr; O1.node_cap = 0; O1.overflow = nullptr;
+        rc = launch(Pr, O1, false, tab, st);
+        if (rc) { release(); return rc; }
+        node_offsets_kernel<<<1, 1024, 0, st>>>(iacc, (int)n, off);
+        TP_TRY(cudaGetLastError());
+        g_launches.fetch_add(1);
+        long long total = 0;
+        TP_TRY(cudaMemcpyAsync(&total, off + n, sizeof(long long), cudaMemcpyDeviceToHost, st));
+        TP_TRY(cudaStreamSynchronize(st));
+        TP_TRY(cudaMallocAsync((void**)&nodes, (size_t)total * NODE_DOUBLES * sizeof(double), st));
+        O1.nodes = nodes; O1.node_offset = off;
+        rc = launch(Pr, O1, false, tab, st);
+        if (rc) { release(); return rc; }
+        node_cap = 0;
+    }
     Outputs O2 = no_outputs();
     O2.images = user.images; O2.nuLnu = user.nuLnu; O2.flag = user.flag; O2.n_attempt = user.n_attempt;
-    O2.nodes = nodes; O2.node_offset = off;
+    O2.nodes = nodes; O2.node_offset = off; O2.node_cap = node_cap; O2.aux_nacc = iacc;
     O2.queue = next_counter(D);
     TP_TRY(cudaMemsetAsync(O2.queue, 0, sizeof(unsigned long long), st));
     if (user.nuLnu) TP_TRY(cudaMemsetAsync(user.nuLnu, 0, sizeof(double) * P.nf, st));

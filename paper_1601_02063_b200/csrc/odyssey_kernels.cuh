@@ -268,9 +268,15 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             // nothing written (its n_accept sizes the node lists).  The ray never ends OPAQUE here.
             if ((commit || fresh) && O.nodes) {
                 RtPoint pt; rt_point<true>(P, L, yn.r, sn, cn, yn.pr, pt);
-                double* nd = O.nodes + NODE_DOUBLES * (O.node_offset[pix] + (long long)(fresh ? 0 : n_acc));
-                nd[0] = fresh ? 0.0 : h_try; nd[1] = pt.fac; nd[2] = pt.E; nd[3] = pt.t0; nd[4] = pt.u0; nd[5] = pt.ycoef;
-                nd[6] = (double)n_att;
+                const long long slot = fresh ? 0 : n_acc;
+                if (O.node_cap > 0 && slot >= O.node_cap) {
+                    *O.overflow = 1;                                       // the caller re-runs with exact sizes
+                } else {
+                    const long long first = O.node_cap > 0 ? (long long)pix * O.node_cap : O.node_offset[pix];
+                    double* nd = O.nodes + NODE_DOUBLES * (first + slot);
+                    nd[0] = fresh ? 0.0 : h_try; nd[1] = pt.fac; nd[2] = pt.E; nd[3] = pt.t0; nd[4] = pt.u0; nd[5] = pt.ycoef;
+                    nd[6] = (double)n_att;
+                }
             }
         } else if (KIND == 2 && (commit || fresh)) {
             RtPoint pt; rt_point<SPEC>(P, L, yn.r, sn, cn, yn.pr, pt);
@@ -396,7 +402,7 @@ __global__ void __launch_bounds__(1024) node_offsets_kernel(const int32_t* __res
 }
 
 template <int G>                                                         // lanes per ray: power of two, nf <= G <= 32
-__global__ void __launch_bounds__(128, 5) spectrum_rt_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs O) {
+__global__ void __launch_bounds__(128, 4) spectrum_rt_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs O) {
     __shared__ double sed[MAX_FREQ];
     for (int k = threadIdx.x; k < MAX_FREQ; k += blockDim.x) sed[k] = 0.0;
     __syncthreads();
@@ -416,8 +422,8 @@ __global__ void __launch_bounds__(128, 5) spectrum_rt_kernel(const __grid_consta
         if (base >= (unsigned long long)npix) break;
         const int pix = (int)base + sub;
         const bool live = pix < npix;
-        const long long off = live ? O.node_offset[pix] : 0;
-        const int cnt = live ? (int)(O.node_offset[pix + 1] - off) : 0;
+        const long long off = !live ? 0 : (O.node_cap > 0 ? (long long)pix * O.node_cap : O.node_offset[pix]);
+        const int cnt = live ? O.aux_nacc[pix] + 1 : 0;
         // a step that ended the ray by capture or escape keeps that flag even if it also made the ray opaque
         // (the fused kernel tests the events before the transfer update); a MAXSTEP ray's last step may end OPAQUE
         const int end_flag = live ? O.aux_flag[pix] : F_MAXSTEP;

@@ -57,6 +57,9 @@ struct Outputs {
     double* nodes;                               // two-phase spectrum path: library scratch, NODE_DOUBLES per node
     const long long* node_offset;                // two-phase spectrum path: first node of each ray, [npix + 1]
     const int32_t* aux_flag;                     // two-phase spectrum path: the record pass's flags (input of phase 2)
+    const int32_t* aux_nacc;                     // two-phase spectrum path: accepted steps per ray (nodes = n_accept + 1)
+    long long node_cap;                          // > 0: fixed capacity, ray's nodes start at pix * node_cap (node_offset unused)
+    int32_t* overflow;                           // record pass: set to 1 when a ray needs more than node_cap nodes
     unsigned long long* queue;                   // work-queue counter (zeroed before the launch)
 };
 

@@ -186,3 +186,47 @@ def test_rk_component_transfer_scheme_matches_the_oracle(ody, orc, nu, tableau):
     # and the two discretisations agree to their truncation error
     a, b = _np(out["image"]).ravel(), _np(base["image"]).ravel()
     assert np.abs(a - b).sum() / b.sum() < 5e-3
+
+
+# ------------------------------------------------------- the two spectrum code paths and the overflow fallback
+def test_spectrum_two_phase_overflow_fallback_matches_the_oracle(ody, orc):
+    """rtol 1e-13: rays take > 511 accepted steps, so the fixed-capacity record pass overflows and the
+    library falls back to count + prefix sum + exact-size record."""
+    w = W.C3(n=12, nf=5, rtol=1e-13)
+    out = ody.render_spectrum(w["scene"], w["model"], w["nu"]); _sync()
+    ref = orc.render_spectrum(w["scene"], w["model"], w["nu"])
+    assert ref["n_attempt"].max() > 600
+    assert np.array_equal(_np(out["flag"]).ravel(), ref["flag"])
+    assert np.mean(_np(out["n_attempt"]).ravel() == ref["n_attempt"]) >= 0.99
+    imgs = _np(out["images"]).reshape(len(w["nu"]), -1)
+    for k in range(len(w["nu"])):
+        _check_image(imgs[k], ref["images"][k], f"overflow fallback k={k}")
+    assert np.allclose(_np(out["nuLnu"]), ref["nuLnu"], rtol=1e-6)
+
+
+def test_fused_spectrum_kernel_on_a_large_image_matches_the_oracle_and_the_two_phase_path(ody, orc):
+    """More rays than four waves of lanes: the fused multi-frequency kernel (accumulators in global scratch)
+    runs instead of the two-phase path.  Checked against the oracle on a strided sub-grid, and against the
+    two-phase path on a sub-image rendered separately with the same pixel centres."""
+    nx, ny, nf = 640, 480, 3
+    sc = W.scene(0.9375, 30.0, nx, 15.0, ny=ny)
+    mo, nu = W.model_riaf(), W.log_spaced_frequencies(1e10, 1e12, nf)
+    out = ody.render_spectrum(sc, mo, nu); _sync()
+    ii = [p * 20 + 10 for q in range(24) for p in range(32)]
+    jj = [q * 20 + 10 for q in range(24) for p in range(32)]
+    ref = orc.render_spectrum(sc, mo, nu, idx=(ii, jj))
+    imgs = _np(out["images"])
+    assert np.array_equal(_np(out["flag"])[jj, ii], ref["flag"])
+    for k in range(nf):
+        _check_image(imgs[k][jj, ii], ref["images"][k], f"fused spectrum k={k}")
+    # SED consistency with the kernel's own images
+    area = (sc["x_max"] - sc["x_min"]) / nx * (sc["y_max"] - sc["y_min"]) / ny
+    rg = orc.rg_cm(mo["mbh_msun"])
+    sed = 4.0 * np.pi * np.asarray(nu) * rg * rg * area * imgs.reshape(nf, -1).sum(axis=1)
+    assert np.allclose(_np(out["nuLnu"]), sed, rtol=1e-10)
+    # the two-phase path on the lower-left 320 x 240 quarter (same pixel centres): identical images
+    sub = dict(sc, nx=320, ny=240, x_max=0.0, y_max=0.0)
+    small = ody.render_spectrum(sub, mo, nu); _sync()
+    a, b = _np(small["images"]), imgs[:, :240, :320]
+    assert np.allclose(a, b, rtol=1e-9, atol=1e-300)
+    assert np.array_equal(_np(small["flag"]), _np(out["flag"])[:240, :320])
