@@ -139,3 +139,37 @@ def test_host_entry_points_match_device_entry_points(ody):
     sh = ody.render_spectrum_host(w3["scene"], w3["model"], w3["nu"])
     assert np.array_equal(_np(s["images"]), sh["images"])
     assert np.allclose(_np(s["nuLnu"]), sh["nuLnu"], rtol=1e-12)
+
+
+def test_concurrent_calls_on_different_streams_do_not_interfere(ody):
+    """Each launch takes its own work-queue counter and passes its constants as kernel parameters, so calls
+    enqueued on different streams may overlap freely."""
+    import torch
+    w2, w0 = W.C2(n=96), W.C0(n=96)
+    ref2 = {k: _np(v).copy() for k, v in ody.render_image(w2["scene"], w2["model"], w2["nu"][0]).items() if v is not None}
+    ref0 = {k: _np(v).copy() for k, v in ody.trace_geodesics(w0["scene"]).items()}
+    _sync()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    for rep in range(4):
+        with torch.cuda.stream(s1):
+            a = ody.render_image(w2["scene"], w2["model"], w2["nu"][0])
+        with torch.cuda.stream(s2):
+            b = ody.trace_geodesics(w0["scene"])
+        outs.append((a, b))
+    _sync()
+    for a, b in outs:
+        for k in ("image", "aux0", "flag", "n_attempt"):
+            assert np.array_equal(_np(a[k]), ref2[k])
+        for k in ref0:
+            assert np.array_equal(_np(b[k]), ref0[k])
+
+
+def test_shutdown_releases_and_library_reinitialises(ody):
+    sc = W.C0(n=16)["scene"]
+    a = {k: _np(v).copy() for k, v in ody.trace_geodesics(sc).items()}
+    _sync()
+    ody.shutdown()
+    b = ody.trace_geodesics(sc); _sync()
+    for k in a:
+        assert np.array_equal(a[k], _np(b[k]))
