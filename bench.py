@@ -45,6 +45,10 @@ UNIT = "ns/photon/step"
 # kernels' arithmetic changes.
 FLOP_PER_ATTEMPT_GEODESIC = 946.6
 FLOP_PER_RT_UPDATE = 397.3
+# DRAM traffic of one launch of the fused kernel on the default workload (C4 at 4096^2), from the same ncu
+# capture: dram__bytes_read.sum + dram__bytes_write.sum = 34.1 MB + 563.8 MB (the outputs are 604 MB; nothing
+# is read but the instruction stream).  Reported only for that workload.
+DRAM_BYTES_PER_LAUNCH_C4_4096 = 34.092800e6 + 563.777280e6
 
 
 def parse_args():
@@ -328,7 +332,9 @@ def run_b200(args):
         "images_per_s": head["images_per_s"],
         "ns_per_photon_per_accepted_step": head["ns_per_photon_per_accepted_step"],
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                     "frac": achieved / peak_tflops, "traffic": None,
+                     "frac": achieved / peak_tflops,
+                     "traffic": DRAM_BYTES_PER_LAUNCH_C4_4096 if (args.model == "riaf" and args.n == 4096 and args.a == 0.998) else None,
+                     "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_c4_riaf_kernel_ncu_full.md)",
                      "kernel": "odyssey_kernel<KIND=%d,TAB=0,SPEC=false>" % mo["kind"], "kernel_ms": kernel_ms,
                      "flop_per_attempt": FLOP_PER_ATTEMPT_GEODESIC, "flop_per_rt_update": flop_rt,
                      "peak_source": "odyssey_fp64_peak_probe (DFMA microbenchmark) in this run, best of 5"},
