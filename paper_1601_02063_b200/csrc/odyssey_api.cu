@@ -208,6 +208,17 @@ int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
     CUDA_TRY(cudaMemsetAsync(O.queue, 0, sizeof(unsigned long long), st));
     if (O.hist && P.nbins > 0) CUDA_TRY(cudaMemsetAsync(O.hist, 0, sizeof(double) * P.nbins, st));
     if (O.nuLnu) CUDA_TRY(cudaMemsetAsync(O.nuLnu, 0, sizeof(double) * P.nf, st));
+    // camera pass: initial state of every queue slot, at full lane efficiency, into stream-ordered scratch
+    double* init_state = nullptr;
+    if (!O.init_state) {
+        CUDA_TRY(cudaMallocAsync((void**)&init_state, sizeof(double) * 6 * (size_t)P.n_queue, st));
+        const long long ib = std::min<long long>((P.n_queue + 255) / 256, (long long)D->n_sm * 16);
+        init_rays_kernel<<<(unsigned)ib, 256, 0, st>>>(P, init_state);
+        cudaError_t ie = cudaGetLastError();
+        if (ie != cudaSuccess) { cudaFreeAsync(init_state, st); return fail(ODYSSEY_ERR_CUDA, "init_rays_kernel: %s", cudaGetErrorString(ie)); }
+        g_launches.fetch_add(1);
+        O.init_state = init_state;
+    }
     if (spec) {      // stream-ordered scratch for the per-frequency accumulators: [5][nf][blocks * nt] doubles
         void* scratch = nullptr;
         CUDA_TRY(cudaMallocAsync(&scratch, sizeof(double) * 5 * (size_t)P.nf * (size_t)blocks * nt, st));
@@ -216,6 +227,7 @@ int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
     void* args[] = {(void*)&P, (void*)&O};
     cudaError_t le = cudaLaunchKernel((const void*)fn, dim3((unsigned)blocks), dim3(nt), args, sm, st);
     if (spec) cudaFreeAsync(O.spec_state, st);
+    if (init_state) cudaFreeAsync(init_state, st);
     if (le != cudaSuccess) return fail(ODYSSEY_ERR_CUDA, "cudaLaunchKernel: %s", cudaGetErrorString(le));
     g_launches.fetch_add(1);
     return ODYSSEY_OK;

@@ -110,9 +110,11 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     const int i = (tile % P.tiles_x) * TILE_W + (w & (TILE_W - 1));
                     const int j = (tile / P.tiles_x) * TILE_H + (w / TILE_W);
                     if (i < P.nx && j < P.ny) {
-                        const double x = P.x_min + (i + 0.5) * P.x_span / P.nx;      // pixel centres (reading K)
-                        const double yy = P.y_min + (j + 0.5) * P.y_span / P.ny;
-                        init_ray(P, x, yy, y, L);
+                        // initial state and L of queue slot q, built at full lane efficiency by init_rays_kernel
+                        // ([6][n_queue] doubles; a refill here runs ~1.5 lanes wide, so no arithmetic is done here)
+                        const double* st = O.init_state + q;
+                        y.r = __ldg(st); y.th = __ldg(st + P.n_queue); y.ph = __ldg(st + 2 * P.n_queue);
+                        y.pr = __ldg(st + 3 * P.n_queue); y.pth = __ldg(st + 4 * P.n_queue); L = __ldg(st + 5 * P.n_queue);
                         pix = j * P.nx + i;
                         n_att = 0; n_acc = 0; mode = M_FRESH; loc_it = 0; on_eq = false;
                         h_try = P.h0; h_next = P.h0; g_disk = 0.0; r_e = 0.0;
@@ -475,6 +477,24 @@ __global__ void __launch_bounds__(128, 4) spectrum_rt_kernel(const __grid_consta
     }
     __syncthreads();
     if (O.nuLnu) for (int q = threadIdx.x; q < nf; q += blockDim.x) if (sed[q] != 0.0) atomicAdd(&O.nuLnu[q], P.sed_coef * P.nu[q] * sed[q]);
+}
+
+// Camera kernel: queue slot q -> pixel (the same 8 x 4 tile mapping as the main kernels) -> initial state and L
+// (§2.2, eqs. (18)-(26), (7), (8), (4), (5)), stored [component][slot] so that both this kernel's
+// stores and the main kernel's refill loads are contiguous per warp.  One thread per slot, every lane busy.
+__global__ void __launch_bounds__(256) init_rays_kernel(const __grid_constant__ Params P, double* __restrict__ state) {
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < P.n_queue; q += (long long)gridDim.x * blockDim.x) {
+        const int tile = (int)(q >> 5), w = (int)(q & 31);
+        const int i = (tile % P.tiles_x) * TILE_W + (w & (TILE_W - 1));
+        const int j = (tile / P.tiles_x) * TILE_H + (w / TILE_W);
+        if (i >= P.nx || j >= P.ny) continue;                            // slot outside a ragged image: never read
+        const double x = P.x_min + (i + 0.5) * P.x_span / P.nx;          // pixel centres (reading K)
+        const double yy = P.y_min + (j + 0.5) * P.y_span / P.ny;
+        State y; double L;
+        init_ray(P, x, yy, y, L);
+        state[q] = y.r; state[q + P.n_queue] = y.th; state[q + 2 * P.n_queue] = y.ph;
+        state[q + 3 * P.n_queue] = y.pr; state[q + 4 * P.n_queue] = y.pth; state[q + 5 * P.n_queue] = L;
+    }
 }
 
 // Diagnostic kernel behind odyssey_eval_math: the device elementary functions, elementwise.

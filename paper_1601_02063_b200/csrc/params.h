@@ -61,6 +61,7 @@ struct Outputs {
     long long node_cap;                          // > 0: fixed capacity, ray's nodes start at pix * node_cap (node_offset unused)
     int32_t* overflow;                           // record pass: set to 1 when a ray needs more than node_cap nodes
     unsigned long long* queue;                   // work-queue counter (zeroed before the launch)
+    const double* init_state;                    // library scratch: initial states by queue slot, [6][n_queue] (init_rays_kernel)
 };
 
 }  // namespace ody
