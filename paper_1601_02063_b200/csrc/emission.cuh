@@ -70,27 +70,24 @@ __constant__ double kK2P[ODY_K2_NC + 1] = { ODY_K2_P(ODY_X) };
 #undef ODY_X
 // 1/K_2(x) = kfac · exp(kexp) for 0 < x; lx = ln x.
 __device__ __forceinline__ void bessel_k2_inv(const double x, const double lx, double& kfac, double& kexp) {
-    if (x <= 2.0) {
-        const double* const ca = kK2A; const double* const cb = kK2B;
-        const double t = 0.25 * x * x;
-        const double lg = lx - 0.69314718055994530942;               // ln(x/2)
-        double A = 0.0, B = 0.0;
+    // Both representations are evaluated and one is selected: in a warp whose lanes sit on both sides of
+    // x = 2 a branch would execute both bodies anyway, one after the other; straight-line code lets the two
+    // (independent) Horner chains interleave.  Neither overflows on the other's domain (x < 700).
+    const double* const ca = kK2A; const double* const cb = kK2B; const double* const cp = kK2P;
+    const double t = 0.25 * x * x;
+    const double z = fma(4.0, d_rcp(x), -1.0);
+    double A = 0.0, B = 0.0, F = 0.0;
 #pragma unroll
-        for (int k = ODY_K2_NS - 1; k >= 0; --k) { A = fma(A, t, ca[k]); B = fma(B, t, cb[k]); }
-        // x² K_2 = 2 − 2t + 4t² (B − ln(x/2) A)
-        const double S = fma(4.0 * t * t, fma(-lg, A, B), fma(-2.0, t, 2.0));
-        kfac = d_rcp(S);
-        kexp = 2.0 * lx;
-    } else {
-        const double* const cp = kK2P;
-        const double z = fma(4.0, d_rcp(x), -1.0);
-        double F = 0.0;
+    for (int k = ODY_K2_NS - 1; k >= 0; --k) { A = fma(A, t, ca[k]); B = fma(B, t, cb[k]); }
 #pragma unroll
-        for (int k = ODY_K2_NC; k >= 0; --k) F = fma(F, z, cp[k]);
-        // K_2 = sqrt(π/2x) e^−x F(z)
-        kfac = d_rcp(F);
-        kexp = x + fma(0.5, lx, -0.22579135264472743236);            // ½ ln(2/π) = −0.2257913526…
-    }
+    for (int k = ODY_K2_NC; k >= 0; --k) F = fma(F, z, cp[k]);
+    const double lg = lx - 0.69314718055994530942;                   // ln(x/2)
+    // x <= 2:  x² K_2 = 2 − 2t + 4t² (B − ln(x/2) A)          ->  1/K_2 = x² / S
+    // x >  2:  K_2 = sqrt(π/2x) e^−x F(z)                       ->  1/K_2 = e^{x + ½ ln x + ½ ln(2/π)} / F
+    const double S = fma(4.0 * t * t, fma(-lg, A, B), fma(-2.0, t, 2.0));
+    const bool small = x <= 2.0;
+    kfac = d_rcp(small ? S : F);
+    kexp = small ? 2.0 * lx : x + fma(0.5, lx, -0.22579135264472743236);
 }
 
 // What all frequencies share at one point of the ray.
