@@ -36,19 +36,20 @@ METRIC = "ns per photon per RK step (FP64)"
 UNIT = "ns/photon/step"
 
 # FP64 work per unit: flop per attempted RK step of the geodesic system, and per
-# radiative-transfer update (one per accepted step, single frequency).  These are the flop the kernels
+# radiative-transfer update (one per accepted step, single frequency).  These are flop the kernels
 # EXECUTE (2 x DFMA + DMUL + DADD thread instructions, predicated on), measured with ncu on this very
-# workload — profiles/r01_c4_geodesic_kernel_ncu_full.md: 946.6 per attempt; profiles/
-# r01_c4_riaf_kernel_ncu_full.md: 1262.0 per attempt with 0.7938 accepted steps per attempt
-# -> (1262.0 - 946.6)/0.7938 = 397.3 per update.  SURVEY.md §8(d)'s a-priori hand count (1500 + ~490)
-# is 58 % higher: it would overstate the achieved rate, so it is not used.  Re-measure when the
-# kernels' arithmetic changes.
-FLOP_PER_ATTEMPT_GEODESIC = 946.6
+# workload: geodesics-only kernel 945.0 per attempt (profiles/r01_c4_geodesic_kernel_ncu_full.md); for the
+# transfer update the LEANEST build measured is used — 397.3 per update ((1262.0 - 946.6)/0.7938, the build
+# before the K_2 branches were replaced by evaluate-both-and-select) — not the 439.8 the final kernel
+# executes (profiles/r01_c4_riaf_kernel_ncu_full.md: 1294.1 per attempt), because the difference is work
+# done only to avoid a divergent branch.  SURVEY.md §8(d)'s a-priori hand count (1500 + ~490) is 58 % higher
+# still: it would overstate the achieved rate, so it is not used.
+FLOP_PER_ATTEMPT_GEODESIC = 945.0
 FLOP_PER_RT_UPDATE = 397.3
 # DRAM traffic of one launch of the fused kernel on the default workload (C4 at 4096^2), from the same ncu
-# capture: dram__bytes_read.sum + dram__bytes_write.sum = 34.1 MB + 563.8 MB (the outputs are 604 MB; nothing
-# is read but the instruction stream).  Reported only for that workload.
-DRAM_BYTES_PER_LAUNCH_C4_4096 = 34.092800e6 + 563.777280e6
+# capture: dram__bytes_read.sum + dram__bytes_write.sum = 842.4 MB + 583.5 MB (805 MB of initial states read,
+# 604 MB of outputs written).  Reported only for that workload.
+DRAM_BYTES_PER_LAUNCH_C4_4096 = 842.362112e6 + 583.544320e6
 
 
 def parse_args():
