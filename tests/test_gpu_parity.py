@@ -173,3 +173,20 @@ def test_shutdown_releases_and_library_reinitialises(ody):
     b = ody.trace_geodesics(sc); _sync()
     for k in a:
         assert np.array_equal(a[k], _np(b[k]))
+
+
+@pytest.mark.parametrize("nx, ny", [(4099, 3), (3, 4099), (1237, 61)])
+def test_extreme_aspect_ratios_and_ragged_tiles_sampled(ody, orc, nx, ny):
+    """Images whose sides are not multiples of the 8 x 4 queue tile, including one-tile-thin strips: every
+    pixel is written exactly once (no NaN / uninitialised values) and a strided sample matches the oracle."""
+    import torch
+    sc = W.scene(0.9, 60.0, nx, 12.0, ny=ny)
+    out = ody.trace_geodesics(sc); _sync()
+    gpu = {k: _np(v) for k, v in out.items()}
+    assert np.isin(gpu["flag"], [W.FLAG_ESCAPED, W.FLAG_CAPTURED]).all()
+    assert (gpu["n_attempt"] > 0).all() and np.isfinite(gpu["theta"]).all()
+    ii = list(range(0, nx, max(nx // 40, 1)))[:40]
+    jj = list(range(0, ny, max(ny // 40, 1)))[:40]
+    I = [i for j in jj for i in ii]; J = [j for j in jj for i in ii]
+    ref = orc.trace_geodesics(sc, idx=(I, J))
+    _check_geodesics(gpu, ref, sel=(np.asarray(I), np.asarray(J)))
