@@ -230,3 +230,34 @@ def test_fused_spectrum_kernel_on_a_large_image_matches_the_oracle_and_the_two_p
     a, b = _np(small["images"]), imgs[:, :240, :320]
     assert np.allclose(a, b, rtol=1e-9, atol=1e-300)
     assert np.array_equal(_np(small["flag"]), _np(out["flag"])[:240, :320])
+
+
+# ------------------------------------------------------------------------------ parameter and edge-case sweep
+@pytest.mark.parametrize("label, scene_kw, model_kw, nu", [
+    ("retrograde spin, Cash-Karp", dict(a=-0.8, incl=50.0, tableau=W.TABLEAU_CASH_KARP), dict(), 230e9),
+    ("near observer r_obs=200 inside the emitting region", dict(a=0.6, incl=70.0, r_obs=200.0), dict(), 86e9),
+    ("j_scale = 4 pi (eq. (37) as printed)", dict(a=0.9375, incl=30.0), dict(j_scale=4.0 * np.pi), 230e9),
+    ("thin flow, strong field", dict(a=0.5, incl=80.0), dict(h_over_r=0.1, beta=1.0, n0=3e7), 345e9),
+    ("cold flow: K_2 large-argument branch everywhere", dict(a=0.9, incl=45.0), dict(T0=3e9, T_index=-0.5), 22e9),
+    ("hot flow: K_2 series everywhere", dict(a=0.9, incl=45.0), dict(T0=3e12, T_index=-0.3, n0=1e5), 230e9),
+    ("small tau_max: most rays end OPAQUE", dict(a=0.9375, incl=30.0), dict(tau_max=0.5), 5e9),
+    ("no electrons: dark image", dict(a=0.3, incl=20.0), dict(n0=0.0), 230e9),
+    ("small emitting region", dict(a=0.998, incl=85.0), dict(r_rt_out=12.0), 230e9),
+    ("face-on", dict(a=0.7, incl=0.5), dict(), 230e9),
+    ("loose tolerance", dict(a=0.9375, incl=30.0, rtol=1e-5), dict(), 230e9),
+])
+def test_riaf_parameter_sweep_matches_the_oracle(ody, orc, label, scene_kw, model_kw, nu):
+    kw = dict(scene_kw)
+    sc = W.scene(kw.pop("a"), kw.pop("incl"), 36, 14.0, **kw)
+    mo = W.model_riaf(**model_kw)
+    out = ody.render_image(sc, mo, nu); _sync()
+    ref = orc.render_image(sc, mo, nu)
+    assert np.array_equal(_np(out["flag"]).ravel(), ref["flag"]), label
+    assert np.mean(_np(out["n_attempt"]).ravel() == ref["n_attempt"]) >= 0.99, label
+    img = _np(out["image"]).ravel()
+    if ref["image"].max() == 0.0:
+        assert np.all(img == 0.0), label
+    else:
+        _check_image(img, ref["image"], label)
+    if "OPAQUE" in label:
+        assert np.mean(ref["flag"] == W.FLAG_OPAQUE) > 0.3
