@@ -65,6 +65,9 @@ def parse_args():
     p.add_argument("--cpu-sample", type=int, default=448, help="side of the strided sub-grid the oracle is timed on")
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
+    p.add_argument("--no-fp32-variant", action="store_true")
+    p.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
+                   help="mixed: time the mixed-precision transfer variant as the main kernel (for ncu captures)")
     return p.parse_args()
 
 
@@ -242,10 +245,11 @@ def run_b200(args):
     # step (weak scaling, no data-path collective — DESIGN.md §9).
     w = workload(args)
     sc, mo, nu = w["scene"], w["model"], w["nu"][0]
-    out = ody.render_image(sc, mo, nu)
+    prec = ody.PREC_MIXED_FP32 if args.precision == "mixed" else ody.PREC_FP64
+    out = ody.render_image(sc, mo, nu, precision=prec)
     torch.cuda.synchronize()
     for _ in range(max(args.warmup - 1, 0)):
-        ody.render_image(sc, mo, nu, out=out)
+        ody.render_image(sc, mo, nu, out=out, precision=prec)
     barrier()
 
     # ---- timed region: exactly K steps, CUDA events on the launching (current) stream
@@ -257,7 +261,7 @@ def run_b200(args):
     barrier()
     ev[0].record()
     for k in range(args.steps):
-        ody.render_image(sc, mo, nu, out=out)
+        ody.render_image(sc, mo, nu, out=out, precision=prec)
         ev[k + 1].record()
     barrier()
     launches = ody.launch_count() - launches0
@@ -283,6 +287,29 @@ def run_b200(args):
         tf = flop / (e0.elapsed_time(e1) * 1e-3) / 1e12
         best = tf if best is None else max(best, tf)
     peak_tflops = best
+
+    # ---- north_star subsystem (c): the mixed-precision (FP32 polynomial cores) transfer variant, same launch
+    # configuration, timed the same way and compared with the FP64 image of the timed steps
+    fp32 = None
+    if args.model == "riaf" and not args.no_fp32_variant and args.precision == "fp64":
+        ref_img = out["image"].clone()
+        out32 = ody.render_image(sc, mo, nu, precision=ody.PREC_MIXED_FP32)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            ody.render_image(sc, mo, nu, out=out32, precision=ody.PREC_MIXED_FP32)
+        e1.record()
+        torch.cuda.synchronize()
+        diff = (out32["image"] - ref_img).abs()
+        l1 = float(diff.sum() / ref_img.sum())
+        mask = ref_img >= 1e-6 * ref_img.max()
+        mx = float((diff[mask] / ref_img[mask]).max())
+        fp32 = {"ms_per_step": e0.elapsed_time(e1) / args.steps, "rel_l1_vs_fp64": l1, "max_rel_vs_fp64": mx,
+                "flags_equal": bool(torch.equal(out32["flag"], out["flag"])),
+                "inside_tolerance": bool(l1 <= 1e-6 and mx <= 1e-4),
+                "what": "FP32 polynomial cores of exp / expm1 / log / K_2 in the transfer block; geodesic, exponent "
+                        "sums and accumulators FP64 (DESIGN.md 8.1)"}
 
     # ---- end to end through the host-buffer C-ABI call (device alloc + kernel + D2H inside the timed region)
     e2e = None
@@ -323,7 +350,7 @@ def run_b200(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
+        "dtype": "f64" if args.precision == "fp64" else "f64 geodesic + f32 transfer cores", "data": "synthetic",
         "config": {"workload": workload_name(args.n, args.a, args.model), "photons_per_step": int(rays_all),
                    "attempted_rk_steps_per_step": int(attempts_all), "accepted_rk_steps_per_step": int(accepts_all),
                    "attempts_per_photon": attempts_all / rays_all,
@@ -345,6 +372,11 @@ def run_b200(args):
         "paper_context": "~1 ns per photon per RK step claimed on a GTX 780 Ti (FP64, geodesics only); "
                          "its Table 1 gives 25732 ms / 1.578e9 steps = 16.3 ns at 1024^2",
     }
+    if fp32:
+        fp32["value"] = fp32["ms_per_step"] * 1e6 / attempts
+        fp32["unit"] = UNIT
+        fp32["speedup_vs_fp64"] = kernel_ms / fp32["ms_per_step"]
+        line["fp32_variant"] = fp32
     if e2e:
         _, d2h, h2d, att_host = e2e
         line["e2e"] = {"value": e2e_s_max / args.steps * 1e9 / (att_host * world), "unit": UNIT,

@@ -61,6 +61,11 @@ enum { ODYSSEY_KIND_NONE = 0, ODYSSEY_KIND_THIN_DISK = 1, ODYSSEY_KIND_RIAF = 2 
  * Runge–Kutta system (coefficients evaluated at all six stages, fifth-order weights, not in the error
  * norm); single-frequency calls only.                                                              */
 enum { ODYSSEY_RT_PER_STEP = 0, ODYSSEY_RT_RK_COMPONENTS = 1 };
+/* FP64: everything in double precision (default).  MIXED_FP32: the geodesic, every exponent sum, argument
+ * reduction and accumulator stay FP64; the polynomial cores of exp / expm1 / log and the K_2 polynomials of the
+ * emissivity run in FP32 (relative error ~1e-7 per coefficient).  Offered for measurement: on B200 it is not
+ * faster.                                                                            */
+enum { ODYSSEY_PREC_FP64 = 0, ODYSSEY_PREC_MIXED_FP32 = 1 };
 #define ODYSSEY_MAX_FREQ 32
 
 /* The observer, the image plane and the integrator controls. */
@@ -94,7 +99,7 @@ typedef struct odyssey_model {
     double g_lo, g_hi;         /* kind 1: histogram range in g                                   */
     double g_power;            /* kind 1: pixel value = g^g_power r_e^-emis_index                */
     int32_t rt_scheme;         /* kind 2: ODYSSEY_RT_* — how eqs. (30), (31) are advanced along the ray */
-    int32_t pad2;
+    int32_t precision;         /* kind 2: ODYSSEY_PREC_* (single-frequency image calls with ODYSSEY_RT_PER_STEP only) */
 } odyssey_model;
 
 /* Geodesics only (BASELINE.json:configs[0]; §2.1-2.2).  Per pixel: outcome flag, the

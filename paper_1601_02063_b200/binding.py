@@ -43,7 +43,7 @@ class Model(C.Structure):
                 ("T0", C.c_double), ("T_index", C.c_double), ("h_over_r", C.c_double), ("beta", C.c_double),
                 ("r_rt_out", C.c_double), ("tau_max", C.c_double), ("j_scale", C.c_double),
                 ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double),
-                ("rt_scheme", C.c_int32), ("pad2", C.c_int32)]
+                ("rt_scheme", C.c_int32), ("precision", C.c_int32)]
 
 
 def _struct(cls, d):
@@ -138,7 +138,10 @@ def trace_geodesics(scene):
     return out
 
 
-def render_image(scene, model, nu_hz=0.0, out=None):
+PREC_FP64, PREC_MIXED_FP32 = 0, 1
+
+
+def render_image(scene, model, nu_hz=0.0, out=None, precision=PREC_FP64):
     """odyssey_render_image: image, aux0, aux1, flag, n_attempt, n_accept ([ny, nx]) and hist ([nbins] or None).
     `out` may carry pre-allocated tensors from a previous call (re-used, e.g. by bench.py)."""
     torch = _torch()
@@ -153,7 +156,9 @@ def render_image(scene, model, nu_hz=0.0, out=None):
                    n_attempt=torch.empty((ny, nx), dtype=torch.int32, device="cuda"),
                    n_accept=torch.empty((ny, nx), dtype=torch.int32, device="cuda"),
                    hist=torch.empty((nb,), **f64) if nb > 0 else None)
-    _check(L.odyssey_render_image(C.byref(_struct(Scene, scene)), C.byref(_struct(Model, model)), C.c_double(nu_hz),
+    mstruct = _struct(Model, model)
+    mstruct.precision = int(precision)
+    _check(L.odyssey_render_image(C.byref(_struct(Scene, scene)), C.byref(mstruct), C.c_double(nu_hz),
                                   _ptr(out["image"]), _ptr(out["aux0"]), _ptr(out["aux1"]), _ptr(out["flag"]),
                                   _ptr(out["n_attempt"]), _ptr(out.get("n_accept")), _ptr(out.get("hist")),
                                   _stream(torch)))

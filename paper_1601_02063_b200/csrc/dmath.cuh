@@ -27,9 +27,11 @@
 #if defined(__CUDACC__)
 #define ODY_HD __device__ __forceinline__
 #define ODY_TABLE __constant__ double
+#define ODY_TABLE_F __constant__ float
 #else
 #define ODY_HD inline
 #define ODY_TABLE static const double
+#define ODY_TABLE_F static const float
 #endif
 
 namespace ody {
@@ -39,6 +41,10 @@ ODY_TABLE kSinS[ODY_SINS_N] = { ODY_SINS(ODY_COEF) };
 ODY_TABLE kCosC[ODY_COSC_N] = { ODY_COSC(ODY_COEF) };
 ODY_TABLE kExpQ[ODY_EXPQ_N] = { ODY_EXPQ(ODY_COEF) };
 ODY_TABLE kLogP[ODY_LOGP_N] = { ODY_LOGP(ODY_COEF) };
+#define ODY_COEFF(i, v) (float)(v),
+ODY_TABLE_F kExpQf[ODY_EXPQF_N] = { ODY_EXPQF(ODY_COEFF) };
+ODY_TABLE_F kLogPf[ODY_LOGPF_N] = { ODY_LOGPF(ODY_COEFF) };
+#undef ODY_COEFF
 // scalar constants that do not fit a 32-bit immediate (low word non-zero)
 ODY_TABLE kDm[10] = {
     6755399441055744.0,             // 0: 1.5 * 2^52, round-to-nearest-integer trick
@@ -209,6 +215,59 @@ ODY_HD double d_expm1_nc(double x) {
 
 // e^x - 1 with the argument clamped to [-700, 700] (e^-700 - 1 = -1 exactly in FP64).
 ODY_HD double d_expm1(double x) { return d_expm1_nc(x < -700.0 ? -700.0 : (x > 700.0 ? 700.0 : x)); }
+
+// ---- mixed-precision variants: argument reduction and reconstruction in FP64 — the integer
+// part of an exponent must not lose bits — and only the polynomial core on the reduced argument in FP32
+// (relative error ~1e-7).  Used by the PREC = 1 transfer code only.
+ODY_HD float f_fmaf(float a, float b, float c) {
+#if defined(__CUDA_ARCH__)
+    return fmaf(a, b, c);
+#else
+    return __builtin_fmaf(a, b, c);
+#endif
+}
+ODY_HD float f_expq(float r) {
+    float p = kExpQf[ODY_EXPQF_N - 1];
+#if defined(__CUDA_ARCH__)
+#pragma unroll
+#endif
+    for (int i = ODY_EXPQF_N - 2; i >= 0; --i) p = f_fmaf(p, r, kExpQf[i]);
+    return p;
+}
+ODY_HD double f_exp_nc(double x) {
+    double two_k;
+    const float r = (float)d_exp_reduce(x, two_k);
+    return d_fma((double)(r * f_expq(r)), two_k, two_k);
+}
+ODY_HD double f_exp(double x) {
+    const bool ok = x >= -700.0;
+    const double v = f_exp_nc(ok ? (x > 700.0 ? 700.0 : x) : -700.0);
+    return ok ? v : 0.0;
+}
+ODY_HD double f_expm1_nc(double x) {
+    double two_k;
+    const float r = (float)d_exp_reduce(x, two_k);
+    return d_fma((double)(r * f_expq(r)), two_k, two_k - 1.0);
+}
+ODY_HD double f_log(double x) {
+    const uint64_t u = d_to_bits(x);
+    const uint64_t adj = u + 0x00095f619980c433ull;
+    const int32_t e = (int32_t)(adj >> 52) - 1023;
+    const float f = (float)(d_from_bits(u - ((uint64_t)(int64_t)e << 52)) - 1.0);
+#if defined(__CUDA_ARCH__)
+    const float s = __fdividef(f, 2.0f + f);
+#else
+    const float s = f / (2.0f + f);
+#endif
+    const float z = s * s;
+    float p = kLogPf[ODY_LOGPF_N - 1];
+#if defined(__CUDA_ARCH__)
+#pragma unroll
+#endif
+    for (int i = ODY_LOGPF_N - 2; i >= 0; --i) p = f_fmaf(p, z, kLogPf[i]);
+    const double ef = (double)e;
+    return d_fma(ef, kDm[7], (double)(2.0f * s * p) + ef * kDm[8]);
+}
 
 // natural logarithm of a normal x > 0.
 ODY_HD double d_log(double x) {

@@ -63,13 +63,42 @@ __device__ __forceinline__ bool flow_igamma(const Params& P, const double L, con
     return true;
 }
 
+// PREC = 0: FP64 throughout.  PREC = 1: the mixed-precision variant of north_star subsystem (c) — exponent sums,
+// argument reductions and accumulators stay FP64, the polynomial cores of exp / expm1 / log and the K_2
+// polynomials run in FP32.
+template <int PREC> __device__ __forceinline__ double p_exp_nc(double x) { return PREC ? f_exp_nc(x) : d_exp_nc(x); }
+template <int PREC> __device__ __forceinline__ double p_exp(double x) { return PREC ? f_exp(x) : d_exp(x); }
+template <int PREC> __device__ __forceinline__ double p_expm1_nc(double x) { return PREC ? f_expm1_nc(x) : d_expm1_nc(x); }
+template <int PREC> __device__ __forceinline__ double p_log(double x) { return PREC ? f_log(x) : d_log(x); }
+
 #define ODY_X(i, v) v,
+#define ODY_XF(i, v) (float)(v),
+__constant__ float kK2Af[ODY_K2_NS] = { ODY_K2_A(ODY_XF) };
+__constant__ float kK2Bf[ODY_K2_NS] = { ODY_K2_B(ODY_XF) };
+__constant__ float kK2Pf[ODY_K2_NC + 1] = { ODY_K2_P(ODY_XF) };
+#undef ODY_XF
 __constant__ double kK2A[ODY_K2_NS] = { ODY_K2_A(ODY_X) };
 __constant__ double kK2B[ODY_K2_NS] = { ODY_K2_B(ODY_X) };
 __constant__ double kK2P[ODY_K2_NC + 1] = { ODY_K2_P(ODY_X) };
 #undef ODY_X
 // 1/K_2(x) = kfac · exp(kexp) for 0 < x; lx = ln x.
+template <int PREC>
 __device__ __forceinline__ void bessel_k2_inv(const double x, const double lx, double& kfac, double& kexp) {
+    if (PREC == 1) {                                                  // same formulas, Horner chains in FP32
+        const float t = (float)(0.25 * x * x), z = (float)fma(4.0, d_rcp(x), -1.0);
+        float A = 0.0f, B = 0.0f, F = 0.0f;
+#pragma unroll
+        for (int k = ODY_K2_NS - 1; k >= 0; --k) { A = fmaf(A, t, kK2Af[k]); B = fmaf(B, t, kK2Bf[k]); }
+#pragma unroll
+        for (int k = ODY_K2_NC; k >= 0; --k) F = fmaf(F, z, kK2Pf[k]);
+        const double lg = lx - 0.69314718055994530942;
+        const double td = 0.25 * x * x;
+        const double S = fma(4.0 * td * td, fma(-lg, (double)A, (double)B), fma(-2.0, td, 2.0));
+        const bool small = x <= 2.0;
+        kfac = d_rcp(small ? S : (double)F);
+        kexp = small ? 2.0 * lx : x + fma(0.5, lx, -0.22579135264472743236);
+        return;
+    }
     // Both representations are evaluated and one is selected: in a warp whose lanes sit on both sides of
     // x = 2 a branch would execute both bodies anyway, one after the other; straight-line code lets the two
     // (independent) Horner chains interleave.  Neither overflows on the other's domain (x < 700).
@@ -102,7 +131,7 @@ struct RtPoint {
 
 // HOIST: evaluate the x_M^(1/12) exponential once per point (spectrum kernel: ν_k^(1/12) is a constant per
 // frequency) instead of once per frequency (single-frequency kernels: same work, fewer live registers).
-template <bool HOIST>
+template <bool HOIST, int PREC = 0>
 __device__ __forceinline__ void rt_point(const Params& P, const double L, const double r, const double s, const double c,
                                          const double pr, RtPoint& q) {
     q.on = false; q.fac = 0.0; q.E = 0.0; q.t0 = 1.0; q.u0 = 1.0; q.lxm0 = 0.0; q.ycoef = 0.0;   // off: every coefficient evaluates to 0
@@ -110,23 +139,23 @@ __device__ __forceinline__ void rt_point(const Params& P, const double L, const 
     double igam;
     if (!flow_igamma(P, L, r, s, c, pr, igam)) return;
     if (!(igam > 0.0) || isinf(igam)) return;
-    const double lr = d_log(r);
+    const double lr = p_log<PREC>(r);
     const double lrel = lr - P.ln_rh;                               // ln(r / r_h)
     const double ln_ne = fma(P.n_index, lrel, fma(-c * c, P.inv_2h2, P.ln_n0));
     const double ln_Th = fma(P.T_index, lrel, P.ln_Theta0);         // ln Θ_e
     if (!(ln_Th > -6.5 && ln_Th < 690.0)) return;                   // 1/Θ_e > 665: K_2 underflows, no emission
     if (!(ln_ne > -1e300)) return;                                  // n0 = 0
-    const double x = d_exp_nc(-ln_Th);                              // 1/Θ_e
+    const double x = p_exp_nc<PREC>(-ln_Th);                        // 1/Θ_e
     double kfac, kexp;
-    bessel_k2_inv(x, -ln_Th, kfac, kexp);
-    const double ligam = d_log(igam);
+    bessel_k2_inv<PREC>(x, -ln_Th, kfac, kexp);
+    const double ligam = p_log<PREC>(igam);
     // ln ν_c = ln nuc_coef + ½ (ln B2_coef + ln n_e − ln r) + 2 ln Θ_e         (eq. (39), B² = B2_coef n_e / r)
     const double ln_nuc = fma(0.5, ln_ne - lr, fma(2.0, ln_Th, P.ln_nuc0));
     q.on = true;
     q.fac = P.rg_cm * kfac;
     q.E = P.ln_j0 + ln_ne + kexp - ligam;
     if (HOIST) {
-        q.t0 = d_exp_nc((ligam - ln_nuc) * (1.0 / 12.0));           // ln(x_M/ν) = ln(1/γ) − ln ν_c; |argument| < 700
+        q.t0 = p_exp_nc<PREC>((ligam - ln_nuc) * (1.0 / 12.0));     // ln(x_M/ν) = ln(1/γ) − ln ν_c; |argument| < 700
         q.u0 = d_rcp(q.t0);
     } else {
         q.lxm0 = ligam - ln_nuc;
@@ -141,32 +170,33 @@ __device__ __forceinline__ void rt_point(const Params& P, const double L, const 
 struct Freq { double nu, ln_nu, nu12, inu12; };
 __device__ __forceinline__ Freq freq_of(const Params& P, const int k) { return Freq{P.nu[k], P.ln_nu[k], P.nu12[k], P.inu12[k]}; }
 
-template <bool HOIST>
+template <bool HOIST, int PREC = 0>
 __device__ __forceinline__ void rt_coefficients(const Params& P, const RtPoint& q, const Freq& f, double& acoef, double& ecoef) {
     const double nu = f.nu, ln_nu = f.ln_nu;
     // straight-line on purpose (no early return when the point is off: fac = 0 gives ε = a = 0), so that the
     // spectrum kernel's unrolled frequency loop can interleave independent chains
     double t, u;                                                     // x_M^(1/12) and its reciprocal
     if (HOIST) { t = q.t0 * f.nu12; u = q.u0 * f.inu12; }
-    else { t = d_exp_nc((ln_nu + q.lxm0) * (1.0 / 12.0)); u = d_rcp(t); }
+    else { t = d_exp_nc((ln_nu + q.lxm0) * (1.0 / 12.0)); u = d_rcp(t); }   // FP64 in both variants: t^4 sits in an exponent
     const double t2 = t * t, u2 = u * u;
     const double u3 = u2 * u;
     const double poly = fma(u3, fma(0.5316, u3, 0.40), 1.0);        // eq. (38) bracket
-    const double ex = d_exp(fma(-1.8899, t2 * t2, fma(-2.0, ln_nu, q.E)));
+    const double ex = p_exp<PREC>(fma(-1.8899, t2 * t2, fma(-2.0, ln_nu, q.E)));
     const double eps = q.fac * u2 * poly * ex;                       // reading D, F
     const double ya = nu * q.ycoef;                                  // hν0/kT_e >= 0
     const bool planck_ok = ya < 700.0;                               // beyond: B_ν underflows, α = 0 as in the formula
-    const double em1 = d_expm1_nc(planck_ok ? ya : 700.0);           // e^{hν0/kT} − 1
+    const double em1 = p_expm1_nc<PREC>(planck_ok ? ya : 700.0);     // e^{hν0/kT} − 1
     ecoef = eps;
     acoef = (eps > 0.0 && planck_ok) ? eps * em1 * P.inv_planck : 0.0;   // Kirchhoff
 }
 
 // Trapezoid in λ for Δτ and the emission, exact attenuation across the step: φ(x) = (1 − e^−x)/x.
+template <int PREC = 0>
 __device__ __forceinline__ void rt_update(const double a0, const double a1, const double e0, const double e1,
                                           const double dl, const double tau_max, double& tau, double& T, double& I) {
     const bool live = !(tau > tau_max);                              // a frozen frequency keeps its values (selects, no branch)
     const double dtau = 0.5 * (a0 + a1) * dl;
-    const double em = d_expm1_nc(dtau < 700.0 ? -dtau : -700.0);     // e^−Δτ − 1 (Δτ >= 0)
+    const double em = p_expm1_nc<PREC>(dtau < 700.0 ? -dtau : -700.0);   // e^−Δτ − 1 (Δτ >= 0)
     const double phi = (dtau > 1e-300) ? -em * d_rcp(dtau) : 1.0;
     const double In = fma(T * (0.5 * (e0 + e1) * dl), phi, I);
     const double Tn = fma(T, em, T);

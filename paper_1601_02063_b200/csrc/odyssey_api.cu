@@ -105,6 +105,10 @@ int check_model(const odyssey_model* M) {
     if (M->kind == ODYSSEY_KIND_RIAF) {
         if (M->rt_scheme != ODYSSEY_RT_PER_STEP && M->rt_scheme != ODYSSEY_RT_RK_COMPONENTS)
             return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown rt_scheme %d", M->rt_scheme);
+        if (M->precision != ODYSSEY_PREC_FP64 && M->precision != ODYSSEY_PREC_MIXED_FP32)
+            return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown precision %d", M->precision);
+        if (M->precision == ODYSSEY_PREC_MIXED_FP32 && M->rt_scheme != ODYSSEY_RT_PER_STEP)
+            return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "precision MIXED_FP32 needs rt_scheme PER_STEP");
         if (!(M->mbh_msun > 0.0) || !(M->h_over_r > 0.0) || !(M->beta > 0.0) || !(M->T0 > 0.0) || !(M->n0 >= 0.0) ||
             !(M->j_scale >= 0.0))
             return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "RIAF parameters mbh_msun, h_over_r, beta, T0 must be positive, n0 and j_scale non-negative");
@@ -153,7 +157,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
         P->ln_j0 = std::log(4.0505 * M->j_scale * kE * kE / (std::sqrt(3.0) * kC));
         P->h_over_mc2 = kH / (kMe * kC * kC);
         P->inv_planck = kC * kC / (2.0 * kH);
-        P->r_rt_out = M->r_rt_out; P->tau_max = M->tau_max; P->rt_scheme = M->rt_scheme;
+        P->r_rt_out = M->r_rt_out; P->tau_max = M->tau_max; P->rt_scheme = M->rt_scheme; P->precision = M->precision;
         P->rg_cm = kGMsun * M->mbh_msun / (kC * kC);
         P->sed_coef = 4.0 * kPi * P->rg_cm * P->rg_cm * P->pix_area;
         for (int k = 0; k < nf && k < MAX_FREQ; ++k) { P->nu[k] = nu[k]; P->ln_nu[k] = std::log(nu[k]); P->nu12[k] = std::exp(P->ln_nu[k] / 12.0); P->inu12[k] = 1.0 / P->nu12[k]; P->nu3[k] = nu[k] * nu[k] * nu[k]; }
@@ -167,7 +171,9 @@ constexpr int NT_SPEC = 128, MINB_SPEC = 3;     // 168 registers (the unrolled f
 
 typedef void (*KernelFn)(const Params, const Outputs);
 
-KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0) {
+KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0, int prec = 0) {
+    if (kind == 2 && !spec && rts == 0 && prec == 1)
+        return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_MAIN, 0, 1> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_MAIN, 0, 1>;
     if (kind == 2 && !spec && rts == 1)
         return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_RK, 1> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_RK, 1>;
     if (kind == 2 && !spec && rts == 2)
@@ -191,7 +197,7 @@ int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
     DevState* D = nullptr;
     int rc = device_state(&D, nullptr);
     if (rc) return rc;
-    KernelFn fn = pick_kernel(P.kind, spec, tab, P.rt_scheme);
+    KernelFn fn = pick_kernel(P.kind, spec, tab, P.rt_scheme, P.precision);
     const int nt = spec ? NT_SPEC : NT_MAIN;
     const size_t sm = smem_bytes(P.kind, spec, P.nf, P.nbins, P.rt_scheme);
     if (sm > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
@@ -393,6 +399,7 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
     if (rc) return rc;
     if (model->kind != ODYSSEY_KIND_RIAF) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode needs model kind 2 (RIAF), got %d", model->kind);
     if (model->rt_scheme != ODYSSEY_RT_PER_STEP) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode supports rt_scheme 0 (per-step update) only");
+    if (model->precision != ODYSSEY_PREC_FP64) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode supports precision FP64 only");
     if (nf < 1 || nf > ODYSSEY_MAX_FREQ) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nf = %d outside [1, %d]", nf, ODYSSEY_MAX_FREQ);
     if (!nu_hz_host) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz_host is NULL");
     for (int k = 0; k < nf; ++k)

@@ -60,7 +60,8 @@ __host__ __device__ constexpr int smem_per_thread(int rts) { return (rts == 1 ? 
 
 // RTS = 1: transfer scheme E' (tau, I as Runge–Kutta components; single frequency only).
 // RTS = 2: record mode, the first phase of the two-phase spectrum path (see spectrum_rt_kernel below).
-template <int KIND, int TAB, bool SPEC, int NT, int MINB, int RTS = 0>
+// PREC = 1: mixed-precision transfer (FP32 polynomial cores; single frequency, per-step scheme only).
+template <int KIND, int TAB, bool SPEC, int NT, int MINB, int RTS = 0, int PREC = 0>
 __global__ void __launch_bounds__(NT, MINB)
 odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs O) {
     extern __shared__ double smem[];
@@ -281,7 +282,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                 }
             }
         } else if (KIND == 2 && (commit || fresh)) {
-            RtPoint pt; rt_point<SPEC>(P, L, yn.r, sn, cn, yn.pr, pt);
+            RtPoint pt; rt_point<SPEC, PREC>(P, L, yn.r, sn, cn, yn.pr, pt);
             bool all_opaque = true;
             if (SPEC) {
 #pragma unroll 4
@@ -297,7 +298,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     ACC(3, k) = a1; ACC(4, k) = e1;
                 }
             } else {
-                double a1, e1; rt_coefficients<false>(P, pt, freq_of(P, 0), a1, e1);
+                double a1, e1; rt_coefficients<false, PREC>(P, pt, freq_of(P, 0), a1, e1);
                 if (commit && RTS == 1) {
                     double tau = RT1(0);
                     if (!(tau > P.tau_max)) {                              // frozen once tau > tau_max
@@ -308,7 +309,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     all_opaque = (tau > P.tau_max);
                 } else if (commit) {
                     double tau = RT1(0), Tr = RT1(1), Inu = RT1(2);
-                    rt_update(RT1(3), a1, RT1(4), e1, h_try, P.tau_max, tau, Tr, Inu);
+                    rt_update<PREC>(RT1(3), a1, RT1(4), e1, h_try, P.tau_max, tau, Tr, Inu);
                     RT1(0) = tau; RT1(1) = Tr; RT1(2) = Inu;
                     all_opaque = (tau > P.tau_max);
                 }
@@ -513,7 +514,7 @@ __global__ void eval_math_kernel(int op, int n, const double* __restrict__ x, do
         case 6: r = d_log(v); break;
         case 8: r = d_rcp_seed(v); break;
         case 9: r = d_rsqrt_seed(v); break;
-        default: { double kf, ke; bessel_k2_inv(v, d_log(v), kf, ke); r = d_rcp(kf) * d_exp(-ke); }
+        default: { double kf, ke; bessel_k2_inv<0>(v, d_log(v), kf, ke); r = d_rcp(kf) * d_exp(-ke); }
     }
     y[i] = r;
     if (y2) y2[i] = r2;

@@ -39,6 +39,7 @@ struct Params {
     double r_rt_out, tau_max, rg_cm;
     double sed_coef;                            // 4π r_g^2 Δx Δy
     int32_t nf, rt_scheme;                      // rt_scheme: ODYSSEY_RT_* (kind 2)
+    int32_t precision, pad3;                    // ODYSSEY_PREC_* (kind 2)
     double nu[MAX_FREQ];
     double ln_nu[MAX_FREQ];
     double nu12[MAX_FREQ], inu12[MAX_FREQ];     // ν^(1/12) and its reciprocal (eq. (38) in powers of x_M^(1/12))

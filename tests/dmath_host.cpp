@@ -12,6 +12,9 @@ void dm_eval(int op, int n, const double* x, double* y, double* y2) {
             case 4: y[i] = ody::d_exp(x[i]); break;
             case 5: y[i] = ody::d_expm1(x[i]); break;
             case 6: y[i] = ody::d_log(x[i]); break;
+            case 10: y[i] = ody::f_exp(x[i]); break;
+            case 11: y[i] = ody::f_expm1_nc(x[i]); break;
+            case 12: y[i] = ody::f_log(x[i]); break;
         }
     }
 }

@@ -65,6 +65,12 @@ def test_invalid_model_and_frequencies_are_rejected():
     bad_rt = B._struct(B.Model, dict(w["model"], rt_scheme=5))
     assert L.odyssey_render_image(C.byref(sc), C.byref(bad_rt), C.c_double(1e9),
                                   None, None, None, None, None, None, None, None) == -1
+    mixed_rk = B._struct(B.Model, dict(w["model"], rt_scheme=W.RT_RK_COMPONENTS)); mixed_rk.precision = 1
+    assert L.odyssey_render_image(C.byref(sc), C.byref(mixed_rk), C.c_double(1e9),
+                                  None, None, None, None, None, None, None, None) == -1
+    mixed = B._struct(B.Model, w["model"]); mixed.precision = 1
+    assert L.odyssey_render_spectrum(C.byref(sc), C.byref(mixed), nu, 4, None, None, None, None, None) == -1
+    assert "precision" in ody.last_error()
     thin = B._struct(B.Model, W.C1()["model"])
     assert L.odyssey_render_spectrum(C.byref(sc), C.byref(thin), nu, 4, None, None, None, None, None) == -1
     assert L.odyssey_render_image(None, None, C.c_double(0.0), None, None, None, None, None, None, None, None) == -1

@@ -261,3 +261,21 @@ def test_riaf_parameter_sweep_matches_the_oracle(ody, orc, label, scene_kw, mode
         _check_image(img, ref["image"], label)
     if "OPAQUE" in label:
         assert np.mean(ref["flag"] == W.FLAG_OPAQUE) > 0.3
+
+
+# ------------------------------------------------------------- mixed-precision transfer variant (north_star (c))
+@pytest.mark.parametrize("nu", [230.0e9, 30.0e9])
+def test_mixed_fp32_transfer_variant_accuracy_against_the_oracle(ody, orc, nu):
+    """The variant is 'reported only if it stays inside tolerance' (north_star): this measures it against the
+    oracle at the same tolerances as the FP64 path — 1e-6 relative L1, 1e-4 max per-pixel relative."""
+    w = W.C2(n=96)
+    out = ody.render_image(w["scene"], w["model"], nu, precision=ody.PREC_MIXED_FP32); _sync()
+    ref = orc.render_image(w["scene"], w["model"], nu)
+    assert np.array_equal(_np(out["flag"]).ravel(), ref["flag"])
+    assert np.array_equal(_np(out["n_attempt"]).ravel() == ref["n_attempt"], _np(out["n_attempt"]).ravel() == ref["n_attempt"])
+    _check_image(_np(out["image"]).ravel(), ref["image"], f"mixed FP32 variant at {nu:g} Hz")
+    # and it really is a different arithmetic: not bit-identical to the FP64 kernel
+    base = ody.render_image(w["scene"], w["model"], nu); _sync()
+    a, b = _np(out["image"]).ravel(), _np(base["image"]).ravel()
+    l1 = np.abs(a - b).sum() / b.sum()
+    assert 1e-10 < l1 < 1e-6
