@@ -227,7 +227,11 @@ int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
     }
     if (spec) {      // stream-ordered scratch for the per-frequency accumulators: [5][nf][blocks * nt] doubles
         void* scratch = nullptr;
-        CUDA_TRY(cudaMallocAsync(&scratch, sizeof(double) * 5 * (size_t)P.nf * (size_t)blocks * nt, st));
+        cudaError_t se = cudaMallocAsync(&scratch, sizeof(double) * 5 * (size_t)P.nf * (size_t)blocks * nt, st);
+        if (se != cudaSuccess) {
+            if (init_state) cudaFreeAsync(init_state, st);
+            return fail(ODYSSEY_ERR_CUDA, "spectrum scratch: %s", cudaGetErrorString(se));
+        }
         O.spec_state = (double*)scratch;
     }
     void* args[] = {(void*)&P, (void*)&O};
@@ -276,11 +280,16 @@ int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st) 
     int32_t* ovf = nullptr;
     TP_TRY(cudaMallocAsync((void**)&ovf, sizeof(int32_t), st));
     TP_TRY(cudaMemsetAsync(ovf, 0, sizeof(int32_t), st));
-    TP_TRY(cudaMallocAsync((void**)&nodes, n * NODE_CAP * NODE_DOUBLES * sizeof(double), st));
-    O1.nodes = nodes; O1.node_cap = NODE_CAP; O1.overflow = ovf;
-    int rc = launch(Pr, O1, false, tab, st);
+    int rc = ODYSSEY_OK;
     int32_t overflow = 0;
-    if (rc == ODYSSEY_OK) {
+    if (cudaMallocAsync((void**)&nodes, n * NODE_CAP * NODE_DOUBLES * sizeof(double), st) != cudaSuccess) {
+        cudaGetLastError();                                                    // no room for fixed-capacity lists:
+        nodes = nullptr; overflow = 1;                                         // size them exactly instead
+    } else {
+        O1.nodes = nodes; O1.node_cap = NODE_CAP; O1.overflow = ovf;
+        rc = launch(Pr, O1, false, tab, st);
+    }
+    if (rc == ODYSSEY_OK && !overflow) {
         cudaError_t e1 = cudaMemcpyAsync(&overflow, ovf, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
         if (e1 == cudaSuccess) e1 = cudaStreamSynchronize(st);                 // the one synchronisation of this path
         if (e1 != cudaSuccess) rc = fail(ODYSSEY_ERR_CUDA, "two-phase spectrum: %s", cudaGetErrorString(e1));
@@ -291,7 +300,8 @@ int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st) 
     if (overflow) {
         // Some ray took more accepted steps than NODE_CAP - 1 (tight tolerances): size the lists exactly —
         // count pass (same kernel, no node buffer), prefix sum, read the total, record again.
-        cudaFreeAsync(nodes, st); nodes = nullptr;
+        if (nodes) cudaFreeAsync(nodes, st);
+        nodes = nullptr;
         O1.nodes = nullptr; O1.node_cap = 0; O1.overflow = nullptr;
         rc = launch(Pr, O1, false, tab, st);
         if (rc) { release(); return rc; }
