@@ -108,10 +108,11 @@ def init_ray(scene, x, y):
     return st, dict(E=cons[0], L=cons[1], Q=cons[2], E2_raw=cons[3], L_raw=cons[4])
 
 
-def rhs(a, E, L, y):
-    y = _vec(y); dy = np.zeros(5)
+def rhs(a, E, L, y, with_t=False):
+    """Slopes of (r, theta, phi, p_r, p_theta); with_t=True appends dt/dlambda of eq. (9)."""
+    y = _vec(y)[:5].copy(); dy = np.zeros(6)
     lib().oracle_rhs(C.c_double(a), C.c_double(E), C.c_double(L), _dp(y), _dp(dy))
-    return dy
+    return dy if with_t else dy[:5]
 
 
 def null_ratio(a, E, L, y):
@@ -191,17 +192,17 @@ def trace_points(scene, model, nu, xs, ys):
     nu = _vec(nu); nf = nu.size
     out = dict(flag=np.zeros(n, np.int32), r=np.zeros(n), th=np.zeros(n), ph=np.zeros(n),
                n_attempt=np.zeros(n, np.int32), n_accept=np.zeros(n, np.int32),
-               g=np.zeros(n), r_e=np.zeros(n), I=np.zeros((n, nf)), tau=np.zeros((n, nf)))
+               g=np.zeros(n), r_e=np.zeros(n), I=np.zeros((n, nf)), tau=np.zeros((n, nf)), t=np.zeros(n))
     lib().oracle_trace_points(C.byref(make_scene(scene)), C.byref(make_model(model)), C.c_int(nf), _dp(nu), C.c_int(n),
                               _dp(xs), _dp(ys), _ip(out["flag"]), _dp(out["r"]), _dp(out["th"]), _dp(out["ph"]),
                               _ip(out["n_attempt"]), _ip(out["n_accept"]), _dp(out["g"]), _dp(out["r_e"]),
-                              _dp(out["I"]), _dp(out["tau"]))
+                              _dp(out["I"]), _dp(out["tau"]), _dp(out["t"]))
     return out
 
 
 def trace_path(scene, model, x, y, max_nodes=20000):
-    """Accepted nodes (r, theta, phi, p_r, p_theta, lambda) of one ray (geodesic and events only)."""
-    nodes = np.zeros((max_nodes, 6)); cons = np.zeros(3); res = np.zeros(3, np.int32)
+    """Accepted nodes (r, theta, phi, p_r, p_theta, lambda, t) of one ray (geodesic and events only)."""
+    nodes = np.zeros((max_nodes, 7)); cons = np.zeros(3); res = np.zeros(3, np.int32)
     n = lib().oracle_trace_path(C.byref(make_scene(scene)), C.byref(make_model(model)), C.c_double(x), C.c_double(y),
                                 C.c_int(max_nodes), _dp(nodes), _dp(cons), _ip(res))
     return nodes[:min(n, max_nodes)], dict(E=cons[0], L=cons[1], Q=cons[2]), dict(flag=int(res[0]), n_attempt=int(res[1]),
@@ -220,10 +221,10 @@ def trace_geodesics(scene, idx=None):
     """C0 driver.  idx = (i_list, j_list) restricts to those pixels; default whole grid, row-major [j][i]."""
     n, ii, jj = _pixels(scene, idx)
     out = dict(flag=np.zeros(n, np.int32), r=np.zeros(n), th=np.zeros(n), ph=np.zeros(n),
-               n_attempt=np.zeros(n, np.int32), n_accept=np.zeros(n, np.int32))
+               n_attempt=np.zeros(n, np.int32), n_accept=np.zeros(n, np.int32), t=np.zeros(n))
     lib().oracle_trace_geodesics(C.byref(make_scene(scene)), C.c_int(n), _ip(ii), _ip(jj),
                                  _ip(out["flag"]), _dp(out["r"]), _dp(out["th"]), _dp(out["ph"]),
-                                 _ip(out["n_attempt"]), _ip(out["n_accept"]))
+                                 _ip(out["n_attempt"]), _ip(out["n_accept"]), _dp(out["t"]))
     return out
 
 

@@ -104,10 +104,11 @@ void circular_orbit_EL(double a, double r, double* E, double* L) {
 // State y = (r, theta, phi, p_r, p_theta)  (t is not needed by any output; PAPER.md:L88 lists it).
 // ----------------------------------------------------------------------------------------------
 struct Ray { double a, E, L, Q; };
+constexpr int NV = 6;      // y = (r, theta, phi, p_r, p_theta, t): the six parameters of PAPER.md:L88; t does not enter the error norm
 
 // Steps 1-4: pixel -> Boyer-Lindquist position, velocity, constants, momenta.  PAPER.md:L104-143.
 // raw[0..1] receive E^2 and L_z BEFORE the |E| normalisation (for the closed-form pins).
-void init_ray(const Scene& S, double x, double y, Ray* ray, double st[5], double raw[2]) {
+void init_ray(const Scene& S, double x, double y, Ray* ray, double st[NV], double raw[2]) {
     const double a = S.a, z = 0.0;
     const double so = std::sin(S.theta_obs), co = std::cos(S.theta_obs);
     const double sp = std::sin(S.phi_obs), cp = std::cos(S.phi_obs);
@@ -146,13 +147,13 @@ void init_ray(const Scene& S, double x, double y, Ray* ray, double st[5], double
     // eq. (13) with mu = 0
     double Q = pth * pth + (L * L / (s * s) - a * a * E * E) * c * c;
     ray->a = a; ray->E = E; ray->L = L; ray->Q = Q;
-    st[0] = r; st[1] = th; st[2] = ph; st[3] = pr; st[4] = pth;
+    st[0] = r; st[1] = th; st[2] = ph; st[3] = pr; st[4] = pth; st[5] = 0.0;   // coordinate time counted from the observer
 }
 
 // Step 5: right-hand side.  rdot, thetadot from (4),(5); phidot (12); pdot_r, pdot_theta are
 // -dH/dr, -dH/dtheta of H = G/(2 Sigma) WITHOUT the null constraint substituted [reading A]; on
 // G = 0 they are eqs. (14),(15).  Pole clamp of PAPER.md:L90 [reading I].
-void rhs(const Ray& ray, const double y[5], double dy[5]) {
+void rhs(const Ray& ray, const double y[NV], double dy[NV]) {
     const double a = ray.a, E = ray.E, L = ray.L;
     const double r = y[0], th = y[1], pr = y[3], pth = y[4];
     double s = std::sin(th), c = std::cos(th);
@@ -168,6 +169,7 @@ void rhs(const Ray& ray, const double y[5], double dy[5]) {
     dy[3] = -((r - 1.0) * pr * pr - 2.0 * r * E * P / Delta + (r - 1.0) * P * P / (Delta * Delta)) / Sigma
             + r * G / (Sigma * Sigma);
     dy[4] = s * c * (L * L / (s * s * s * s) - a * a * E * E) / Sigma - a * a * s * c * G / (Sigma * Sigma);
+    dy[5] = E + (2.0 * r * (r * r + a * a) * E - 2.0 * a * r * L) / (Sigma * Delta);                      // eq. (9)
 }
 
 // Scale-free null-condition residual [reading R]: G over the sum of the magnitudes of its terms.
@@ -227,11 +229,11 @@ Tableau make_tableau(int which) {
 // One attempt of size h from y: 5th-order result ynew and the error estimate yerr = 5th - 4th,
 // formed as h * sum (b5_j - b4_j) k_j exactly as Press et al.'s rkck does.
 // ystage (optional) receives the six stage states y + h sum_j A_ij k_j.
-void rk_attempt(const Ray& ray, const Tableau& T, const double y[5], double h, double ynew[5], double yerr[5],
-                double (*ystage)[5] = nullptr) {
-    double k[6][5], ytmp[5];
+void rk_attempt(const Ray& ray, const Tableau& T, const double y[NV], double h, double ynew[NV], double yerr[NV],
+                double (*ystage)[NV] = nullptr) {
+    double k[6][NV], ytmp[NV];
     for (int i = 0; i < 6; ++i) {
-        for (int v = 0; v < 5; ++v) {
+        for (int v = 0; v < NV; ++v) {
             double acc = 0.0;
             for (int j = 0; j < i; ++j) acc += T.A[i][j] * k[j][v];
             ytmp[v] = y[v] + h * acc;
@@ -239,7 +241,7 @@ void rk_attempt(const Ray& ray, const Tableau& T, const double y[5], double h, d
         }
         rhs(ray, ytmp, k[i]);
     }
-    for (int v = 0; v < 5; ++v) {
+    for (int v = 0; v < NV; ++v) {
         double s5 = 0.0, se = 0.0;
         for (int j = 0; j < 6; ++j) { s5 += T.b5[j] * k[j][v]; se += (T.b5[j] - T.b4[j]) * k[j][v]; }
         ynew[v] = y[v] + h * s5;
@@ -248,7 +250,7 @@ void rk_attempt(const Ray& ray, const Tableau& T, const double y[5], double h, d
 }
 
 // Step 7: scaled max-norm of the error in units of rtol [reading G].
-double error_norm(const double y[5], const double yerr[5], double rtol) {
+double error_norm(const double y[NV], const double yerr[NV], double rtol) {     // over (r, theta, phi, p_r, p_theta) only
     const double sc[5] = {std::fabs(y[0]), 1.0, 1.0, 1.0 + std::fabs(y[3]), 1.0 + std::fabs(y[4])};
     double e = 0.0;
     for (int v = 0; v < 5; ++v) {
@@ -414,18 +416,18 @@ void rt_rk_step(const Tableau& T, const double a[6], const double eps[6], double
 // Step 8 + the per-ray driver.
 // ----------------------------------------------------------------------------------------------
 struct RayOut {
-    int flag; double r, th, ph; int n_attempt, n_accept;
+    int flag; double r, th, ph, t; int n_attempt, n_accept;
     double g, r_e;                       // thin disk
     std::vector<double> I, tau;          // invariant intensity I_nu/nu^3 and optical depth per frequency
 };
 
-struct Path { std::vector<double> nodes; };   // per accepted node: the 5 state components and the affine parameter
+struct Path { std::vector<double> nodes; };   // per accepted node: (r, theta, phi, p_r, p_theta), the affine parameter, t
 
 constexpr int LOCATE_MAX = 8;
 
 void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double x, double yimg,
                RayOut* out, Path* path) {
-    Ray ray; double y[5];
+    Ray ray; double y[NV];
     init_ray(S, x, yimg, &ray, y, nullptr);
     const Tableau T = make_tableau(S.tableau);
     const Flow F = make_flow(S.a);
@@ -438,11 +440,11 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
     double g = 0.0, r_e = 0.0;
     if (M.kind == 2) rt_coefficients(S, M, F, ray, y, nf, nu, a0.data(), e0.data());
     double lambda = 0.0;
-    if (path) { path->nodes.insert(path->nodes.end(), y, y + 5); path->nodes.push_back(lambda); }
+    if (path) { path->nodes.insert(path->nodes.end(), y, y + 5); path->nodes.push_back(lambda); path->nodes.push_back(y[5]); }
 
     while (flag < 0) {
         if (n_attempt >= S.max_attempts) { flag = MAXSTEP; break; }
-        double ynew[5], yerr[5], ystage[6][5];
+        double ynew[NV], yerr[NV], ystage[6][NV];
         rk_attempt(ray, T, y, h, ynew, yerr, ystage);
         ++n_attempt;
         double err = error_norm(y, yerr, S.rtol);
@@ -462,7 +464,7 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
             for (int it = 0; it < LOCATE_MAX; ++it) {
                 double f = ynew[comp] - target;
                 if (std::fabs(f) <= ftol) break;
-                double dy[5];
+                double dy[NV];
                 rhs(ray, ynew, dy);
                 h_used -= f / dy[comp];
                 rk_attempt(ray, T, y, h_used, ynew, yerr, ystage);
@@ -478,7 +480,7 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
                 flag = DISK;
                 r_e = ynew[0];
                 double u[4];
-                double yeq[5] = {ynew[0], 0.5 * PI, ynew[2], ynew[3], ynew[4]};
+                double yeq[NV] = {ynew[0], 0.5 * PI, ynew[2], ynew[3], ynew[4], ynew[5]};
                 if (flow_velocity(S.a, F, r_e, 0.5 * PI, u)) g = gamma_shift(ray, yeq, u);
             }
         } else {
@@ -512,12 +514,12 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
             }
             if (flag < 0 && all_opaque) flag = OPAQUE;
         }
-        for (int v = 0; v < 5; ++v) y[v] = ynew[v];
+        for (int v = 0; v < NV; ++v) y[v] = ynew[v];
         h = h_next;
         lambda += h_used;
-        if (path) { path->nodes.insert(path->nodes.end(), y, y + 5); path->nodes.push_back(lambda); }
+        if (path) { path->nodes.insert(path->nodes.end(), y, y + 5); path->nodes.push_back(lambda); path->nodes.push_back(y[5]); }
     }
-    out->flag = flag; out->r = y[0]; out->th = y[1]; out->ph = y[2];
+    out->flag = flag; out->r = y[0]; out->th = y[1]; out->ph = y[2]; out->t = y[5];
     out->n_attempt = n_attempt; out->n_accept = n_accept;
     out->g = g; out->r_e = r_e;
     out->I = I; out->tau = tau;
@@ -565,14 +567,17 @@ void oracle_kerr_constants(double a, double* out) {
 
 // st = (r, theta, phi, p_r, p_theta); cons = {E, L, Q, E2_raw, L_raw}
 void oracle_init_ray(const Scene* S, double x, double y, double* st, double* cons) {
-    Ray ray; double raw[2];
-    init_ray(*S, x, y, &ray, st, raw);
+    Ray ray; double raw[2]; double st6[NV];
+    init_ray(*S, x, y, &ray, st6, raw);
+    for (int v = 0; v < 5; ++v) st[v] = st6[v];
     cons[0] = ray.E; cons[1] = ray.L; cons[2] = ray.Q; cons[3] = raw[0]; cons[4] = raw[1];
 }
 
+// y[5] in, dy[6] out: (r, theta, phi, p_r, p_theta) and, last, dt/dlambda of eq. (9)
 void oracle_rhs(double a, double E, double L, const double* y, double* dy) {
     Ray ray{a, E, L, 0.0};
-    rhs(ray, y, dy);
+    double y6[NV] = {y[0], y[1], y[2], y[3], y[4], 0.0};
+    rhs(ray, y6, dy);
 }
 
 double oracle_null_ratio(double a, double E, double L, const double* y) {
@@ -595,17 +600,22 @@ void oracle_tableau(int which, double* c, double* A, double* b5, double* b4) {
 void oracle_rk_attempt(double a, double E, double L, int which, const double* y, double h, double* ynew, double* yerr) {
     Ray ray{a, E, L, 0.0};
     Tableau T = make_tableau(which);
-    rk_attempt(ray, T, y, h, ynew, yerr);
+    double y6[NV] = {y[0], y[1], y[2], y[3], y[4], 0.0}, yn[NV], ye[NV];
+    rk_attempt(ray, T, y6, h, yn, ye);
+    for (int v = 0; v < 5; ++v) { ynew[v] = yn[v]; yerr[v] = ye[v]; }
 }
 
-double oracle_error_norm(const double* y, const double* yerr, double rtol) { return error_norm(y, yerr, rtol); }
+double oracle_error_norm(const double* y, const double* yerr, double rtol) {
+    double y6[NV] = {y[0], y[1], y[2], y[3], y[4], 0.0}, e6[NV] = {yerr[0], yerr[1], yerr[2], yerr[3], yerr[4], 0.0};
+    return error_norm(y6, e6, rtol);
+}
 
 // u[4] = (ut, ur, utheta, uphi); returns 1 if the flow has a velocity there; *gamma = eq. (2).
 int oracle_flow_gamma(double a, double r, double th, double pr, double pth, double L, double* u, double* gamma) {
     Flow F = make_flow(a);
     if (!flow_velocity(a, F, r, th, u)) { *gamma = 0.0; return 0; }
     Ray ray{a, -1.0, L, 0.0};
-    double y[5] = {r, th, 0.0, pr, pth};
+    double y[NV] = {r, th, 0.0, pr, pth, 0.0};
     *gamma = gamma_shift(ray, y, u);
     return 1;
 }
@@ -640,7 +650,7 @@ void oracle_trace_points(const Scene* S, const Model* M, int nf, const double* n
                          const double* xs, const double* ys,
                          int32_t* flag, double* r, double* th, double* ph,
                          int32_t* n_attempt, int32_t* n_accept,
-                         double* g, double* r_e, double* I, double* tau) {
+                         double* g, double* r_e, double* I, double* tau, double* t) {
 #pragma omp parallel for schedule(dynamic, 16)
     for (int k = 0; k < n; ++k) {
         RayOut R;
@@ -653,6 +663,7 @@ void oracle_trace_points(const Scene* S, const Model* M, int nf, const double* n
         if (n_accept) n_accept[k] = R.n_accept;
         if (g) g[k] = R.g;
         if (r_e) r_e[k] = R.r_e;
+        if (t) t[k] = R.t;
         for (int q = 0; q < nf; ++q) {
             if (I) I[(size_t)k * nf + q] = R.I[q];
             if (tau) tau[(size_t)k * nf + q] = R.tau[q];
@@ -660,18 +671,18 @@ void oracle_trace_points(const Scene* S, const Model* M, int nf, const double* n
     }
 }
 
-// Accepted nodes of one ray: nodes[max_nodes][6] = (r, theta, phi, p_r, p_theta, lambda); returns the number of nodes (start included);
+// Accepted nodes of one ray: nodes[max_nodes][7] = (r, theta, phi, p_r, p_theta, lambda, t); returns the number of nodes (start included);
 // cons = {E, L, Q}; res = {flag, n_attempt, n_accept}.
 int oracle_trace_path(const Scene* S, const Model* M, double x, double y, int max_nodes, double* nodes,
                       double* cons, int32_t* res) {
-    Ray ray; double st[5];
+    Ray ray; double st[NV];
     init_ray(*S, x, y, &ray, st, nullptr);
     cons[0] = ray.E; cons[1] = ray.L; cons[2] = ray.Q;
     RayOut R; Path P;
     trace_ray(*S, *M, 0, nullptr, x, y, &R, &P);
-    int n = (int)(P.nodes.size() / 6);
+    int n = (int)(P.nodes.size() / 7);
     int m = std::min(n, max_nodes);
-    std::memcpy(nodes, P.nodes.data(), sizeof(double) * 6 * (size_t)m);
+    std::memcpy(nodes, P.nodes.data(), sizeof(double) * 7 * (size_t)m);
     res[0] = R.flag; res[1] = R.n_attempt; res[2] = R.n_accept;
     return n;
 }
@@ -682,7 +693,7 @@ int oracle_trace_path(const Scene* S, const Model* M, double x, double y, int ma
 // Geodesics only (C0).
 void oracle_trace_geodesics(const Scene* S, int n, const int32_t* idx_i, const int32_t* idx_j,
                             int32_t* flag, double* r, double* th, double* ph,
-                            int32_t* n_attempt, int32_t* n_accept) {
+                            int32_t* n_attempt, int32_t* n_accept, double* t) {
     Model M; std::memset(&M, 0, sizeof(M));
 #pragma omp parallel for schedule(dynamic, 16)
     for (int k = 0; k < n; ++k) {
@@ -692,6 +703,7 @@ void oracle_trace_geodesics(const Scene* S, int n, const int32_t* idx_i, const i
         trace_ray(*S, M, 0, nullptr, x, y, &R, nullptr);
         flag[k] = R.flag; r[k] = R.r; th[k] = R.th; ph[k] = R.ph;
         n_attempt[k] = R.n_attempt; n_accept[k] = R.n_accept;
+        if (t) t[k] = R.t;
     }
 }
 

@@ -160,3 +160,65 @@ def test_against_independent_8_component_hamiltonian_integration(a, incl, x, y):
     assert K.hamilton_rhs(a, end[1], end[2], end[4], end[5], end[6], end[7])[6] == pytest.approx(0.0, abs=1e-10)
     assert out["th"][0] == pytest.approx(end[2], abs=2e-8)
     assert out["ph"][0] == pytest.approx(end[3], abs=2e-8)
+
+
+# ---- coordinate time, eq. (9) (the sixth of the six parameters of PAPER.md:L88) -------------------------
+@pytest.mark.parametrize("a,incl,x,y", [(0.9, 60.0, -5.0, 3.0), (0.998, 85.0, 7.5, 0.5), (0.5, 30.0, 2.0, -6.5)])
+def test_coordinate_time_against_independent_8_component_integration(a, incl, x, y):
+    """t integrated with eq. (9) along the ray equals t of the independent Hamiltonian integration (dt/dlambda =
+    dH/dp_t there).  E = -1: the ray is traced backwards, so t runs to negative values."""
+    sc = W.scene(a, incl, 64, 10.0, rtol=1e-11)
+    st, cons = O.init_ray(sc, x, y)
+    out = O.trace_points(sc, W.model_none(), [], [x], [y])
+
+    def f(lam, s):
+        t, r, th, ph, pt, pr, pth, pph = s
+        d = K.hamilton_rhs(a, r, th, pt, pr, pth, pph)
+        return [d[0], d[1], d[2], d[3], 0.0, d[4], d[5], 0.0]
+
+    def reached(lam, s):
+        return s[1] - sc["r_esc"] if s[5] > 0 else -1.0
+    reached.terminal, reached.direction = True, 1.0
+    s0 = [0.0, st[0], st[1], st[2], -cons["E"], st[3], st[4], cons["L"]]
+    sol = solve_ivp(f, [0.0, 5000.0], s0, method="DOP853", rtol=1e-12, atol=1e-14, events=reached)
+    end = sol.y_events[0][0]
+    assert out["t"][0] < -1900.0
+    assert out["t"][0] == pytest.approx(end[0], abs=2e-7)
+
+
+def test_eq9_slope_equals_hamilton_equation_for_t():
+    rng = np.random.default_rng(3)
+    for _ in range(40):
+        a = rng.uniform(-0.99, 0.99); r = rng.uniform(2.2, 40.0); th = rng.uniform(0.2, 2.9)
+        L = rng.uniform(-6, 6); pr = rng.uniform(-1, 1); pth = rng.uniform(-4, 4)
+        dy = O.rhs(a, -1.0, L, [r, th, 0.0, pr, pth], with_t=True)
+        d = K.hamilton_rhs(a, r, th, 1.0, pr, pth, L)       # p_t = -E = +1
+        assert dy[5] == pytest.approx(d[0], rel=1e-12)
+
+
+@pytest.mark.parametrize("b0", [6.0, 20.0, 150.0])
+def test_schwarzschild_travel_time_equals_orbit_integral(b0):
+    """a = 0, equatorial: elapsed coordinate time between the start radius and r_esc equals the textbook
+    integral  dt = dr / ((1 - 2/r) sqrt(1 - b^2 (1 - 2/r)/r^2))  (two legs, tanh-sinh quadrature); for large b
+    it is the straight-line time plus the first-order (Shapiro) delay
+    2 ln[(r1 + sqrt(r1^2 - b^2))(r2 + sqrt(r2^2 - b^2))/b^2] + sqrt((r1 - b)/(r1 + b)) + sqrt((r2 - b)/(r2 + b))."""
+    sc = W.scene(0.0, 90.0, 64, 10.0, rtol=1e-11)
+    st, cons = O.init_ray(sc, b0, 0.0)
+    b = abs(cons["L"])
+    out = O.trace_points(sc, W.model_none(), [], [b0], [0.0])
+    assert out["flag"][0] == W.FLAG_ESCAPED
+    with mpmath.workdps(30):
+        bb = mpmath.mpf(b)
+        rp = max(z.real for z in mpmath.polyroots([1, 0, -bb ** 2, 2 * bb ** 2], maxsteps=200, extraprec=200))
+        # r = rp + s^2 removes the inverse-square-root singularity at the periastron
+        def leg(r_end):
+            g = lambda s: 2 * s / ((1 - 2 / (rp + s * s)) * mpmath.sqrt(abs(1 - bb ** 2 * (1 - 2 / (rp + s * s)) / (rp + s * s) ** 2)))
+            return mpmath.quad(g, [0, mpmath.sqrt(mpmath.mpf(r_end) - rp)])
+        want = float(leg(st[0]) + leg(out["r"][0]))
+    assert -out["t"][0] == pytest.approx(want, rel=1e-9)
+    if b0 >= 150.0:
+        r1, r2 = st[0], out["r"][0]
+        straight = math.sqrt(r1 * r1 - b * b) + math.sqrt(r2 * r2 - b * b)
+        s1, s2 = math.sqrt(r1 * r1 - b * b), math.sqrt(r2 * r2 - b * b)
+        shapiro = 2.0 * math.log((r1 + s1) * (r2 + s2) / (b * b)) + math.sqrt((r1 - b) / (r1 + b)) + math.sqrt((r2 - b) / (r2 + b))
+        assert -out["t"][0] - straight == pytest.approx(shapiro, rel=2e-2)
