@@ -201,7 +201,8 @@ def test_schwarzschild_travel_time_equals_orbit_integral(b0):
     """a = 0, equatorial: elapsed coordinate time between the start radius and r_esc equals the textbook
     integral  dt = dr / ((1 - 2/r) sqrt(1 - b^2 (1 - 2/r)/r^2))  (two legs, tanh-sinh quadrature); for large b
     it is the straight-line time plus the first-order (Shapiro) delay
-    2 ln[(r1 + sqrt(r1^2 - b^2))(r2 + sqrt(r2^2 - b^2))/b^2] + sqrt((r1 - b)/(r1 + b)) + sqrt((r2 - b)/(r2 + b))."""
+    2 ln[(r1 + sqrt(r1^2 - r0^2))(r2 + sqrt(r2^2 - r0^2))/r0^2] + sqrt((r1 - r0)/(r1 + r0)) + sqrt((r2 - r0)/(r2 + r0)),
+    r0 the periastron."""
     sc = W.scene(0.0, 90.0, 64, 10.0, rtol=1e-11)
     st, cons = O.init_ray(sc, b0, 0.0)
     b = abs(cons["L"])
@@ -217,8 +218,8 @@ def test_schwarzschild_travel_time_equals_orbit_integral(b0):
         want = float(leg(st[0]) + leg(out["r"][0]))
     assert -out["t"][0] == pytest.approx(want, rel=1e-9)
     if b0 >= 150.0:
-        r1, r2 = st[0], out["r"][0]
-        straight = math.sqrt(r1 * r1 - b * b) + math.sqrt(r2 * r2 - b * b)
-        s1, s2 = math.sqrt(r1 * r1 - b * b), math.sqrt(r2 * r2 - b * b)
-        shapiro = 2.0 * math.log((r1 + s1) * (r2 + s2) / (b * b)) + math.sqrt((r1 - b) / (r1 + b)) + math.sqrt((r2 - b) / (r2 + b))
+        r1, r2, r0 = st[0], out["r"][0], float(rp)            # Weinberg's first-order formula is in the periastron r0
+        s1, s2 = math.sqrt(r1 * r1 - r0 * r0), math.sqrt(r2 * r2 - r0 * r0)
+        straight = s1 + s2
+        shapiro = 2.0 * math.log((r1 + s1) * (r2 + s2) / (r0 * r0)) + math.sqrt((r1 - r0) / (r1 + r0)) + math.sqrt((r2 - r0) / (r2 + r0))
         assert -out["t"][0] - straight == pytest.approx(shapiro, rel=2e-2)
