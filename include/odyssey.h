@@ -103,10 +103,12 @@ typedef struct odyssey_model {
 } odyssey_model;
 
 /* Geodesics only (BASELINE.json:configs[0]; §2.1-2.2).  Per pixel: outcome flag, the
- * final Boyer–Lindquist position (r, theta, phi) — located on the stopping surface — and the
+ * final Boyer–Lindquist position (r, theta, phi) — located on the stopping surface — the coordinate
+ * time t elapsed along the ray (eq. (9); counted from 0 at the image plane, negative because
+ * the ray is traced backwards; integrated only when t is non-NULL, never part of the error norm) and the
  * number of attempted and accepted Runge–Kutta steps ("total number of steps").  */
 int odyssey_trace_geodesics(const odyssey_scene* scene,
-                            int32_t* flag, double* r, double* theta, double* phi,
+                            int32_t* flag, double* r, double* theta, double* phi, double* t,
                             int32_t* n_attempt, int32_t* n_accept, void* cuda_stream);
 
 /* One observed frequency nu_hz (ignored by kind 0/1).
@@ -135,7 +137,7 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
 
 /* Host-buffer variants: identical semantics, every output pointer is HOST memory, synchronous. */
 int odyssey_trace_geodesics_host(const odyssey_scene* scene,
-                                 int32_t* flag, double* r, double* theta, double* phi,
+                                 int32_t* flag, double* r, double* theta, double* phi, double* t,
                                  int32_t* n_attempt, int32_t* n_accept);
 int odyssey_render_image_host(const odyssey_scene* scene, const odyssey_model* model, double nu_hz,
                               double* image, double* aux0, double* aux1, int32_t* flag,

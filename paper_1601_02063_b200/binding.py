@@ -74,11 +74,11 @@ def load_library():
     except OSError as e:
         raise OdysseyError(f"cannot load {path}: {e}") from e
     vp, dp, ip = C.c_void_p, C.c_void_p, C.c_void_p
-    L.odyssey_trace_geodesics.argtypes = [C.POINTER(Scene), ip, dp, dp, dp, ip, ip, vp]
+    L.odyssey_trace_geodesics.argtypes = [C.POINTER(Scene), ip, dp, dp, dp, dp, ip, ip, vp]
     L.odyssey_render_image.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.c_double, dp, dp, dp, ip, ip, ip, dp, vp]
     L.odyssey_render_spectrum.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.POINTER(C.c_double), C.c_int,
                                           dp, dp, ip, ip, vp]
-    L.odyssey_trace_geodesics_host.argtypes = [C.POINTER(Scene), ip, dp, dp, dp, ip, ip]
+    L.odyssey_trace_geodesics_host.argtypes = [C.POINTER(Scene), ip, dp, dp, dp, dp, ip, ip]
     L.odyssey_render_image_host.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.c_double, dp, dp, dp, ip, ip, ip, dp]
     L.odyssey_render_spectrum_host.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.POINTER(C.c_double), C.c_int,
                                                dp, dp, ip, ip]
@@ -122,8 +122,8 @@ def _np_ptr(a):
     return C.c_void_p(a.ctypes.data) if a is not None else None
 
 
-def trace_geodesics(scene):
-    """odyssey_trace_geodesics: flag, r, theta, phi, n_attempt, n_accept as [ny, nx] CUDA tensors."""
+def trace_geodesics(scene, with_time=False):
+    """odyssey_trace_geodesics: flag, r, theta, phi, n_attempt, n_accept (and t with with_time) as [ny, nx] CUDA tensors."""
     torch = _torch()
     L = load_library()
     ny, nx = scene["ny"], scene["nx"]
@@ -132,8 +132,10 @@ def trace_geodesics(scene):
     out = dict(flag=torch.empty((ny, nx), **i32), r=torch.empty((ny, nx), **f64), theta=torch.empty((ny, nx), **f64),
                phi=torch.empty((ny, nx), **f64), n_attempt=torch.empty((ny, nx), **i32),
                n_accept=torch.empty((ny, nx), **i32))
+    if with_time:
+        out["t"] = torch.empty((ny, nx), **f64)
     _check(L.odyssey_trace_geodesics(C.byref(_struct(Scene, scene)), _ptr(out["flag"]), _ptr(out["r"]),
-                                     _ptr(out["theta"]), _ptr(out["phi"]), _ptr(out["n_attempt"]),
+                                     _ptr(out["theta"]), _ptr(out["phi"]), _ptr(out.get("t")), _ptr(out["n_attempt"]),
                                      _ptr(out["n_accept"]), _stream(torch)))
     return out
 
@@ -182,13 +184,15 @@ def render_spectrum(scene, model, nu_hz):
     return out
 
 
-def trace_geodesics_host(scene):
+def trace_geodesics_host(scene, with_time=False):
     L = load_library()
     ny, nx = scene["ny"], scene["nx"]
     out = dict(flag=np.empty((ny, nx), np.int32), r=np.empty((ny, nx)), theta=np.empty((ny, nx)), phi=np.empty((ny, nx)),
                n_attempt=np.empty((ny, nx), np.int32), n_accept=np.empty((ny, nx), np.int32))
+    if with_time:
+        out["t"] = np.empty((ny, nx))
     _check(L.odyssey_trace_geodesics_host(C.byref(_struct(Scene, scene)), _np_ptr(out["flag"]), _np_ptr(out["r"]),
-                                          _np_ptr(out["theta"]), _np_ptr(out["phi"]), _np_ptr(out["n_attempt"]),
+                                          _np_ptr(out["theta"]), _np_ptr(out["phi"]), _np_ptr(out.get("t")), _np_ptr(out["n_attempt"]),
                                           _np_ptr(out["n_accept"])))
     return out
 

@@ -18,11 +18,12 @@
 namespace ody {
 
 struct State { double r, th, ph, pr, pth; };     // y of PAPER.md:L88 without t
-struct Slope { double r, th, ph, pr, pth; };     // dy/dλ
+struct Slope { double r, th, ph, pr, pth, t; };  // dy/dλ; t (eq. (9)) is formed only by kernels that output time
 
 // ------------------------------------------------------------------------------------------------
 // Right-hand side.  Also returns sinθ, cosθ (unclamped) for the emission code.
 // ------------------------------------------------------------------------------------------------
+template <bool TIME = false>
 __device__ __forceinline__ void geodesic_rhs(const double a, const double a2, const double L,
                                              const double r, const double th, const double pr, const double pth,
                                              Slope& k, double& sin_th, double& cos_th) {
@@ -45,7 +46,9 @@ __device__ __forceinline__ void geodesic_rhs(const double a, const double a2, co
     const double GiS = G * iS;
     k.r = Delta * pr * iS;                                        // eq. (4)
     k.th = pth * iS;                                              // eq. (5)
-    k.ph = fma(fma(-2.0, r, Sigma) * L, is2, -2.0 * a * r) * (iS * iD);   // eq. (12)
+    const double iSD = iS * iD;
+    k.ph = fma(fma(-2.0, r, Sigma) * L, is2, -2.0 * a * r) * iSD;         // eq. (12)
+    if (TIME) k.t = -fma(2.0 * r * Pm, iSD, 1.0);                         // eq. (9) with E = −1: −1 − 2r(r² + a² + aL)/(ΣΔ)
     k.pr = iS * fma(1.0 - r, fma(q, q, pr2), r * fma(2.0, q, GiS));
     k.pth = (s * c) * iS * fma(-a2, GiS, fma(L * L, is2 * is2, -a2));
 }

@@ -171,7 +171,9 @@ constexpr int NT_SPEC = 128, MINB_SPEC = 3;     // 168 registers (the unrolled f
 
 typedef void (*KernelFn)(const Params, const Outputs);
 
-KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0, int prec = 0) {
+KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0, int prec = 0, bool time = false) {
+    if (kind == 0 && time)
+        return tab ? odyssey_kernel<0, 1, false, NT_MAIN, MINB_MAIN, 0, 0, 1> : odyssey_kernel<0, 0, false, NT_MAIN, MINB_MAIN, 0, 0, 1>;
     if (kind == 2 && !spec && rts == 0 && prec == 1)
         return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_MAIN, 0, 1> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_MAIN, 0, 1>;
     if (kind == 2 && !spec && rts == 1)
@@ -197,7 +199,7 @@ int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
     DevState* D = nullptr;
     int rc = device_state(&D, nullptr);
     if (rc) return rc;
-    KernelFn fn = pick_kernel(P.kind, spec, tab, P.rt_scheme, P.precision);
+    KernelFn fn = pick_kernel(P.kind, spec, tab, P.rt_scheme, P.precision, O.t != nullptr);
     const int nt = spec ? NT_SPEC : NT_MAIN;
     const size_t sm = smem_bytes(P.kind, spec, P.nf, P.nbins, P.rt_scheme);
     if (sm > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
@@ -376,13 +378,13 @@ struct Scratch {
 // ================================================================================================
 extern "C" {
 
-int odyssey_trace_geodesics(const odyssey_scene* scene, int32_t* flag, double* r, double* theta, double* phi,
+int odyssey_trace_geodesics(const odyssey_scene* scene, int32_t* flag, double* r, double* theta, double* phi, double* t,
                             int32_t* n_attempt, int32_t* n_accept, void* cuda_stream) {
     int rc = check_scene(scene);
     if (rc) return rc;
     Params P; fill_params(*scene, nullptr, nullptr, 0, &P);
     Outputs O = no_outputs();
-    O.flag = flag; O.r = r; O.th = theta; O.ph = phi; O.n_attempt = n_attempt; O.n_accept = n_accept;
+    O.flag = flag; O.r = r; O.th = theta; O.ph = phi; O.t = t; O.n_attempt = n_attempt; O.n_accept = n_accept;
     return launch(P, O, false, scene->tableau, (cudaStream_t)cuda_stream);
 }
 
@@ -428,14 +430,14 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
 
 // ---- host-buffer variants (Scratch defined above) ---------------------------------------------
 
-int odyssey_trace_geodesics_host(const odyssey_scene* scene, int32_t* flag, double* r, double* theta, double* phi,
+int odyssey_trace_geodesics_host(const odyssey_scene* scene, int32_t* flag, double* r, double* theta, double* phi, double* t,
                                  int32_t* n_attempt, int32_t* n_accept) {
     TRY(check_scene(scene));
     const size_t n = (size_t)scene->nx * scene->ny;
-    Scratch S; int32_t *dflag, *datt, *dacc; double *dr, *dth, *dph;
-    TRY(S.add(flag, n, &dflag)); TRY(S.add(r, n, &dr)); TRY(S.add(theta, n, &dth)); TRY(S.add(phi, n, &dph));
+    Scratch S; int32_t *dflag, *datt, *dacc; double *dr, *dth, *dph, *dt;
+    TRY(S.add(flag, n, &dflag)); TRY(S.add(r, n, &dr)); TRY(S.add(theta, n, &dth)); TRY(S.add(phi, n, &dph)); TRY(S.add(t, n, &dt));
     TRY(S.add(n_attempt, n, &datt)); TRY(S.add(n_accept, n, &dacc));
-    TRY(odyssey_trace_geodesics(scene, dflag, dr, dth, dph, datt, dacc, nullptr));
+    TRY(odyssey_trace_geodesics(scene, dflag, dr, dth, dph, dt, datt, dacc, nullptr));
     return S.copy_back();
 }
 

@@ -61,7 +61,8 @@ __host__ __device__ constexpr int smem_per_thread(int rts) { return (rts == 1 ? 
 // RTS = 1: transfer scheme E' (tau, I as Runge–Kutta components; single frequency only).
 // RTS = 2: record mode, the first phase of the two-phase spectrum path (see spectrum_rt_kernel below).
 // PREC = 1: mixed-precision transfer (FP32 polynomial cores; single frequency, per-step scheme only).
-template <int KIND, int TAB, bool SPEC, int NT, int MINB, int RTS = 0, int PREC = 0>
+// TIME = 1: also integrate the coordinate time t of eq. (9) (it is not in the error norm) and write it to O.t.
+template <int KIND, int TAB, bool SPEC, int NT, int MINB, int RTS = 0, int PREC = 0, int TIME = 0>
 __global__ void __launch_bounds__(NT, MINB)
 odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs O) {
     extern __shared__ double smem[];
@@ -88,6 +89,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     StagesSmem<NT> K;
     K.base = smem + threadIdx.x;
     double kph0 = 0.0;                                              // φ slope of the cached first stage
+    double y_t = 0.0, kt0 = 0.0;                                    // (TIME) coordinate time and its cached first slope
     double L = 0.0, h_try = 0.0, h_next = 0.0, cos_y = 0.0;
     double g_disk = 0.0, r_e = 0.0;
     y.r = y.th = y.ph = y.pr = y.pth = 0.0;
@@ -117,7 +119,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                         y.r = __ldg(st); y.th = __ldg(st + P.n_queue); y.ph = __ldg(st + 2 * P.n_queue);
                         y.pr = __ldg(st + 3 * P.n_queue); y.pth = __ldg(st + 4 * P.n_queue); L = __ldg(st + 5 * P.n_queue);
                         pix = j * P.nx + i;
-                        n_att = 0; n_acc = 0; mode = M_FRESH; loc_it = 0; on_eq = false;
+                        n_att = 0; n_acc = 0; mode = M_FRESH; loc_it = 0; on_eq = false; y_t = 0.0;
                         h_try = P.h0; h_next = P.h0; g_disk = 0.0; r_e = 0.0;
                         if (KIND == 2) {
                             if (SPEC) {
@@ -144,6 +146,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         bool done = false;                                             // end state evaluated: go on to events / commit
         double ph5 = kRkB5[TAB][0] * kph0;
         double phe = kRkBE[TAB][0] * kph0;
+        double t5 = TIME ? kRkB5[TAB][0] * kt0 : 0.0;
         // scheme E': running fifth-order sums of a and of eps exp(-tau) over the stages; stage 0 = cached start values
         double rk_tau = 0.0, rk_I = 0.0, tau_n = 0.0;
         if (RTS == 1) {
@@ -193,7 +196,12 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                 }
             }
             if (ev) {
-                geodesic_rhs(a, a2, L, ir, ith, ipr, ipth, k, sn, cn);
+                geodesic_rhs<TIME != 0>(a, a2, L, ir, ith, ipr, ipth, k, sn, cn);
+                if (TIME && s < 6) {
+                    const double b5s = (s == 1) ? kRkB5[TAB][1] : (s == 2) ? kRkB5[TAB][2] : (s == 3) ? kRkB5[TAB][3]
+                                     : (s == 4) ? kRkB5[TAB][4] : kRkB5[TAB][5];
+                    t5 = fma(b5s, k.t, t5);
+                }
                 if (RTS == 1 && s < 6) {                                   // coefficients at this stage state
                     RtPoint pt; rt_point<false>(P, L, ir, sn, cn, ipr, pt);
                     double as, es; rt_coefficients<false>(P, pt, freq_of(P, 0), as, es);
@@ -319,6 +327,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         }
         if (commit || fresh) {                                         // (fresh: yn = y)
             y = yn; cos_y = cn; kph0 = kn.ph;
+            if (TIME) { if (commit) y_t = fma(h_try, t5, y_t); kt0 = kn.t; }
             K.set(0, 0, kn.r); K.set(1, 0, kn.th); K.set(2, 0, kn.pr); K.set(3, 0, kn.pth);
             if (commit) h_try = h_next; else mode = M_NORMAL;
         }
@@ -329,6 +338,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             if (O.r) O.r[pix] = y.r;
             if (O.th) O.th[pix] = y.th;
             if (O.ph) O.ph[pix] = y.ph;
+            if (TIME && O.t) O.t[pix] = y_t;
             if (O.n_attempt) O.n_attempt[pix] = n_att;
             if (O.n_accept) O.n_accept[pix] = n_acc;
             if (KIND == 0) {

@@ -49,7 +49,7 @@ struct Params {
 // Output pointers (device memory, any may be null).
 struct Outputs {
     int32_t* flag;
-    double* r; double* th; double* ph;
+    double* r; double* th; double* ph; double* t;
     int32_t* n_attempt; int32_t* n_accept;
     double* image; double* aux0; double* aux1;   // single-frequency image modes
     double* hist;                                // kind 1

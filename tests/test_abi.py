@@ -42,7 +42,7 @@ def test_struct_layout_matches_header_sizes():
 def test_invalid_scene_is_rejected_before_any_cuda_call(patch, msg):
     L = ody.load_library()
     sc = dict(W.C0()["scene"]); sc.update(patch)
-    rc = L.odyssey_trace_geodesics(C.byref(B._struct(B.Scene, sc)), None, None, None, None, None, None, None)
+    rc = L.odyssey_trace_geodesics(C.byref(B._struct(B.Scene, sc)), None, None, None, None, None, None, None, None)
     assert rc == -1
     assert msg in ody.last_error()
 

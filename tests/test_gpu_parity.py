@@ -190,3 +190,25 @@ def test_extreme_aspect_ratios_and_ragged_tiles_sampled(ody, orc, nx, ny):
     I = [i for j in jj for i in ii]; J = [j for j in jj for i in ii]
     ref = orc.trace_geodesics(sc, idx=(I, J))
     _check_geodesics(gpu, ref, sel=(np.asarray(I), np.asarray(J)))
+
+
+@pytest.mark.parametrize("a, incl", [(0.0, 60.0), (0.9, 60.0), (0.998, 85.0)])
+def test_coordinate_time_output_matches_the_oracle(ody, orc, a, incl):
+    """t of eq. (9) along each ray (the sixth parameter of PAPER.md:L88), integrated only on request."""
+    sc = W.scene(a, incl, 48, 10.0)
+    out = ody.trace_geodesics(sc, with_time=True); _sync()
+    gpu = {k: _np(v) for k, v in out.items()}
+    ref = orc.trace_geodesics(sc)
+    _check_geodesics(gpu, ref)
+    t, tr = gpu["t"].ravel(), ref["t"]
+    assert np.all(t < 0.0)
+    esc = ref["flag"] == W.FLAG_ESCAPED
+    assert np.max(np.abs(t[esc] - tr[esc]) / np.abs(tr[esc])) <= 1e-8
+    # captured rays: t diverges logarithmically at the horizon; the stopping radius is located, so it still agrees
+    assert np.max(np.abs(t[~esc] - tr[~esc]) / np.abs(tr[~esc])) <= 1e-7
+    # the other outputs do not depend on whether t is integrated
+    plain = ody.trace_geodesics(sc); _sync()
+    for k in ("flag", "r", "theta", "phi", "n_attempt", "n_accept"):
+        assert np.array_equal(_np(plain[k]), gpu[k])
+    host = ody.trace_geodesics_host(sc, with_time=True)
+    assert np.array_equal(host["t"], gpu["t"])
