@@ -31,7 +31,8 @@ class Model(C.Structure):
                 ("T_index", C.c_double), ("h_over_r", C.c_double), ("beta", C.c_double),
                 ("r_rt_out", C.c_double), ("tau_max", C.c_double), ("j_scale", C.c_double),
                 ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double),
-                ("rt_scheme", C.c_int32), ("pad", C.c_int32)]
+                ("rt_scheme", C.c_int32), ("pad", C.c_int32),
+                ("spot_r_orbit", C.c_double), ("spot_size", C.c_double), ("spot_phi0", C.c_double)]
 
 
 def _fill(struct, d):
@@ -237,6 +238,20 @@ def render_image(scene, model, nu_hz=0.0, idx=None):
     lib().oracle_render_image(C.byref(make_scene(scene)), C.byref(make_model(model)), C.c_double(nu_hz), C.c_int(n),
                               _ip(ii), _ip(jj), _dp(out["image"]), _dp(out["aux0"]), _dp(out["aux1"]),
                               _ip(out["flag"]), _ip(out["n_attempt"]), _ip(out["n_accept"]), _dp(out["hist"]))
+    return out
+
+
+def render_hotspot(scene, model, t_obs, idx=None):
+    n, ii, jj = _pixels(scene, idx)
+    t = _vec(t_obs); nt = t.size
+    nb = int(model.get("nbins", 0))
+    out = dict(images=np.zeros((nt, n)), lightcurve=np.zeros(nt), spectrogram=np.zeros((nt, nb)) if nb > 0 else None,
+               g=np.zeros(n), r_e=np.zeros(n), phi_e=np.zeros(n), t_e=np.zeros(n),
+               flag=np.zeros(n, np.int32), n_attempt=np.zeros(n, np.int32))
+    lib().oracle_render_hotspot(C.byref(make_scene(scene)), C.byref(make_model(model)), _dp(t), C.c_int(nt), C.c_int(n),
+                                _ip(ii), _ip(jj), _dp(out["images"]), _dp(out["lightcurve"]), _dp(out["spectrogram"]),
+                                _dp(out["g"]), _dp(out["r_e"]), _dp(out["phi_e"]), _dp(out["t_e"]),
+                                _ip(out["flag"]), _ip(out["n_attempt"]))
     return out
 
 

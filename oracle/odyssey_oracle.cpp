@@ -75,6 +75,7 @@ struct Model {           // mirrors workloads.model_*()
     double mbh_msun, n0, n_index, T0, T_index, h_over_r, beta, r_rt_out, tau_max, j_scale;
     double g_lo, g_hi, g_power;
     int32_t rt_scheme, pad;  // 0: one update per accepted step [reading E]; 1: tau, I as Runge-Kutta components [E']
+    double spot_r_orbit, spot_size, spot_phi0;   // kind 3 [reading HS]: orbit radius (<= 0: r_isco), r_spot, azimuth at t = 0
 };
 
 // ----------------------------------------------------------------------------------------------
@@ -473,7 +474,7 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
         };
 
         // (1) thin disk: equatorial crossing inside the step [reading P]
-        if (M.kind == 1 && !on_equator && std::cos(y[1]) * std::cos(ynew[1]) < 0.0) {
+        if ((M.kind == 1 || M.kind == 3) && !on_equator && std::cos(y[1]) * std::cos(ynew[1]) < 0.0) {
             locate(1, 0.5 * PI);
             on_equator = true;
             if (ynew[0] >= r_in && ynew[0] <= M.r_out && ynew[0] > r_cap) {
@@ -534,6 +535,24 @@ inline void pixel_xy(const Scene& S, int i, int j, double* x, double* y) {   // 
 double disk_value(const Model& M, const RayOut& R) {
     if (R.flag != DISK || !(R.g > 0.0)) return 0.0;
     return std::pow(R.g, M.g_power) * std::pow(R.r_e, -M.emis_index);
+}
+
+// Kind 3 [reading HS of PAPER.md:L252-264, eq. (36), Figs. 7, 8]: a hot spot on the opaque equatorial plane.
+// Its centre moves on the prograde circular orbit of radius r_s with Omega_s = 1/(r_s^{3/2} + a),
+// phi_s(t) = phi_0 + Omega_s t.  A ray that reaches the plane at (r_e, phi_e) after the coordinate time t_e
+// (negative: the ray is traced backwards from the image plane, where t = 0) left it at t_em = t_obs + t_e; the
+// surface brightness there is g^p exp(-d^2 / 2 r_spot^2) for d < 4 r_spot, d the distance to the spot centre
+// at t_em in the pseudo-Cartesian coordinates of eqs. (33), (34), and 0 otherwise.
+double hot_spot_value(const Scene& S, const Model& M, const RayOut& R, double t_obs) {
+    if (R.flag != DISK || !(R.g > 0.0)) return 0.0;
+    const double a = S.a;
+    const double rs = (M.spot_r_orbit > 0.0) ? M.spot_r_orbit : isco_radius(a);
+    const double Omega = 1.0 / (rs * std::sqrt(rs) + a);
+    const double phi_s = M.spot_phi0 + Omega * (t_obs + R.t);
+    const double Re = std::sqrt(R.r_e * R.r_e + a * a), Rs = std::sqrt(rs * rs + a * a);
+    const double d2 = Re * Re + Rs * Rs - 2.0 * Re * Rs * std::cos(R.ph - phi_s);
+    if (!(d2 < 16.0 * M.spot_size * M.spot_size)) return 0.0;
+    return std::pow(R.g, M.g_power) * std::exp(-d2 / (2.0 * M.spot_size * M.spot_size));
 }
 
 }  // namespace
@@ -736,6 +755,42 @@ void oracle_render_image(const Scene* S, const Model* M, double nu_hz, int n, co
             int b = (int)std::floor((g - M->g_lo) / (M->g_hi - M->g_lo) * M->nbins);
             if (b >= M->nbins) b = M->nbins - 1;
             hist[b] += image[k] * area;
+        }
+    }
+}
+
+// Hot spot (kind 3): images [nt][n], lightcurve[nt] = sum(image) * pixel area, spectrogram [nt][nbins] over g
+// (only when the whole grid is rendered); per pixel g, r_e, phi_e, t_e of the disk crossing.
+void oracle_render_hotspot(const Scene* S, const Model* M, const double* t_obs, int nt, int n,
+                           const int32_t* idx_i, const int32_t* idx_j,
+                           double* images, double* lightcurve, double* spectrogram,
+                           double* g, double* r_e, double* phi_e, double* t_e, int32_t* flag, int32_t* n_attempt) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int k = 0; k < n; ++k) {
+        int i = idx_i ? idx_i[k] : k % S->nx, j = idx_j ? idx_j[k] : k / S->nx;
+        double x, y; pixel_xy(*S, i, j, &x, &y);
+        RayOut R;
+        trace_ray(*S, *M, 0, nullptr, x, y, &R, nullptr);
+        for (int q = 0; q < nt; ++q) images[(size_t)q * n + k] = hot_spot_value(*S, *M, R, t_obs[q]);
+        bool hit = (R.flag == DISK);
+        g[k] = R.g; r_e[k] = R.r_e; phi_e[k] = hit ? R.ph : 0.0; t_e[k] = hit ? R.t : 0.0;
+        flag[k] = R.flag; n_attempt[k] = R.n_attempt;
+    }
+    double area = ((S->x_max - S->x_min) / S->nx) * ((S->y_max - S->y_min) / S->ny);
+    for (int q = 0; q < nt; ++q) {
+        double sum = 0.0;
+        for (int k = 0; k < n; ++k) sum += images[(size_t)q * n + k];
+        if (lightcurve) lightcurve[q] = sum * area;
+        if (spectrogram && M->nbins > 0) {
+            double* h = spectrogram + (size_t)q * M->nbins;
+            for (int b = 0; b < M->nbins; ++b) h[b] = 0.0;
+            for (int k = 0; k < n; ++k) {
+                double v = images[(size_t)q * n + k];
+                if (v == 0.0 || !(g[k] >= M->g_lo && g[k] < M->g_hi)) continue;
+                int b = (int)std::floor((g[k] - M->g_lo) / (M->g_hi - M->g_lo) * M->nbins);
+                if (b >= M->nbins) b = M->nbins - 1;
+                h[b] += v * area;
+            }
         }
     }
 }

@@ -18,7 +18,7 @@ import math
 # Flags written per ray (same numbering on both sides; it is part of the output contract).
 FLAG_ESCAPED, FLAG_CAPTURED, FLAG_DISK, FLAG_OPAQUE, FLAG_MAXSTEP = 0, 1, 2, 3, 4
 
-KIND_NONE, KIND_THIN_DISK, KIND_RIAF = 0, 1, 2
+KIND_NONE, KIND_THIN_DISK, KIND_RIAF, KIND_HOT_SPOT = 0, 1, 2, 3
 # How eqs. (30), (31) are advanced (readings E, E'): one exact-attenuation update per accepted
 # step (default), or tau and I as two more Runge-Kutta components through the six stages.
 RT_PER_STEP, RT_RK_COMPONENTS = 0, 1
@@ -40,7 +40,8 @@ def model_none():
     return dict(kind=KIND_NONE, r_in=0.0, r_out=0.0, emis_index=0.0,
                 mbh_msun=0.0, n0=0.0, n_index=0.0, T0=0.0, T_index=0.0, h_over_r=1.0, beta=1.0,
                 r_rt_out=0.0, tau_max=0.0, j_scale=1.0,
-                nbins=0, g_lo=0.0, g_hi=1.0, g_power=0.0, rt_scheme=RT_PER_STEP)
+                nbins=0, g_lo=0.0, g_hi=1.0, g_power=0.0, rt_scheme=RT_PER_STEP,
+                spot_r_orbit=0.0, spot_size=0.0, spot_phi0=0.0)
 
 
 def model_thin_disk(r_in=0.0, r_out=50.0, emis_index=3.0, nbins=200, g_lo=0.0, g_hi=2.0, g_power=3.0):
@@ -49,6 +50,15 @@ def model_thin_disk(r_in=0.0, r_out=50.0, emis_index=3.0, nbins=200, g_lo=0.0, g
     m = model_none()
     m.update(kind=KIND_THIN_DISK, r_in=float(r_in), r_out=float(r_out), emis_index=float(emis_index),
              nbins=int(nbins), g_lo=float(g_lo), g_hi=float(g_hi), g_power=float(g_power))
+    return m
+
+
+def model_hot_spot(r_orbit=0.0, r_spot=0.5, phi0=0.0, r_in=0.0, r_out=50.0, g_power=4.0, nbins=100, g_lo=0.0, g_hi=2.0):
+    """Keplerian hot spot on the opaque equatorial plane (eq. (36)): Gaussian of width r_spot
+    = 0.5 r_g, cut at 4 r_spot, orbiting at r_orbit (<= 0: r_isco of the scene's spin), azimuth phi0 at t = 0."""
+    m = model_none()
+    m.update(kind=KIND_HOT_SPOT, r_in=float(r_in), r_out=float(r_out), g_power=float(g_power), nbins=int(nbins),
+             g_lo=float(g_lo), g_hi=float(g_hi), spot_r_orbit=float(r_orbit), spot_size=float(r_spot), spot_phi0=float(phi0))
     return m
 
 
