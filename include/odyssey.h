@@ -54,7 +54,7 @@ enum {
 };
 
 enum { ODYSSEY_TABLEAU_RKF45 = 0, ODYSSEY_TABLEAU_CASH_KARP = 1 };
-enum { ODYSSEY_KIND_NONE = 0, ODYSSEY_KIND_THIN_DISK = 1, ODYSSEY_KIND_RIAF = 2 };
+enum { ODYSSEY_KIND_NONE = 0, ODYSSEY_KIND_THIN_DISK = 1, ODYSSEY_KIND_RIAF = 2, ODYSSEY_KIND_HOT_SPOT = 3 };
 /* PAPER.md:L171 says the transfer equations are "easily integrated along with the geodesic … piecewise
  * according to these steps".  PER_STEP (default): one update per accepted step, trapezoid in lambda with
  * the exact attenuation across the step.  RK_COMPONENTS: tau and I as two more components of the
@@ -100,6 +100,9 @@ typedef struct odyssey_model {
     double g_power;            /* kind 1: pixel value = g^g_power r_e^-emis_index                */
     int32_t rt_scheme;         /* kind 2: ODYSSEY_RT_* — how eqs. (30), (31) are advanced along the ray */
     int32_t precision;         /* kind 2: ODYSSEY_PREC_* (single-frequency image calls with ODYSSEY_RT_PER_STEP only) */
+    double spot_r_orbit;       /* kind 3: radius of the spot's circular equatorial orbit; <= 0 means r_isco(a)  */
+    double spot_size;          /* kind 3: r_spot of eq. (36) (the paper uses 0.5 r_g); emission is cut at 4 r_spot */
+    double spot_phi0;          /* kind 3: azimuth of the spot centre at coordinate time t = 0                    */
 } odyssey_model;
 
 /* Geodesics only (BASELINE.json:configs[0]; §2.1-2.2).  Per pixel: outcome flag, the
@@ -135,6 +138,20 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
                             double* images, double* nuLnu, int32_t* flag, int32_t* n_attempt,
                             void* cuda_stream);
 
+/* Orbiting hot spot (§4.4, eq. (36), Figs. 7-8; kind 3, which also uses kind 1's r_in, r_out,
+ * g_power, nbins, g_lo, g_hi).  The spot is a Gaussian patch, exp(-d^2 / 2 spot_size^2) for d < 4 spot_size, on the
+ * opaque equatorial plane; its centre moves on the prograde circular orbit of radius spot_r_orbit,
+ * phi_s(t) = spot_phi0 + t / (r_s^{3/2} + a).  A ray that reaches the plane at (r_e, phi_e) after the coordinate
+ * time t_e (eq. (9); negative, the ray is traced backwards from t = 0 at the image plane) shows the spot as it was
+ * at t_obs + t_e; d is measured in the pseudo-Cartesian coordinates of eqs. (33), (34).  For each of the nt <= 32
+ * observer times t_obs_host[k] (HOST memory): images[k][ny][nx] = g^g_power exp(-d^2/2 spot_size^2),
+ * lightcurve[k] = sum(images[k]) x pixel area, spectrogram[k][nbins] = that flux binned over g (NULL or nbins = 0:
+ * skipped).  Per pixel: g, r_e, phi_e, t_e of the crossing (0 where the ray misses the plane), flag, n_attempt. */
+int odyssey_render_hotspot(const odyssey_scene* scene, const odyssey_model* model, const double* t_obs_host, int nt,
+                           double* images, double* lightcurve, double* spectrogram,
+                           double* g, double* r_e, double* phi_e, double* t_e, int32_t* flag, int32_t* n_attempt,
+                           void* cuda_stream);
+
 /* Host-buffer variants: identical semantics, every output pointer is HOST memory, synchronous. */
 int odyssey_trace_geodesics_host(const odyssey_scene* scene,
                                  int32_t* flag, double* r, double* theta, double* phi, double* t,
@@ -145,6 +162,9 @@ int odyssey_render_image_host(const odyssey_scene* scene, const odyssey_model* m
 int odyssey_render_spectrum_host(const odyssey_scene* scene, const odyssey_model* model,
                                  const double* nu_hz_host, int nf,
                                  double* images, double* nuLnu, int32_t* flag, int32_t* n_attempt);
+int odyssey_render_hotspot_host(const odyssey_scene* scene, const odyssey_model* model, const double* t_obs_host, int nt,
+                                double* images, double* lightcurve, double* spectrogram,
+                                double* g, double* r_e, double* phi_e, double* t_e, int32_t* flag, int32_t* n_attempt);
 
 /* FP64 peak probe (BASELINE.json:north_star "measured by a DFMA microbenchmark in the same run"):
  * enqueues a kernel in which every thread runs `iters` rounds of 16 independent DFMA chains

@@ -16,8 +16,9 @@ import numpy as np
 from . import build as _build
 
 EXPORTED_SYMBOLS = (
-    "odyssey_trace_geodesics", "odyssey_render_image", "odyssey_render_spectrum",
+    "odyssey_trace_geodesics", "odyssey_render_image", "odyssey_render_spectrum", "odyssey_render_hotspot",
     "odyssey_trace_geodesics_host", "odyssey_render_image_host", "odyssey_render_spectrum_host",
+    "odyssey_render_hotspot_host",
     "odyssey_fp64_peak_probe", "odyssey_kernel_info", "odyssey_eval_math", "odyssey_launch_count",
     "odyssey_last_error", "odyssey_shutdown",
 )
@@ -43,7 +44,8 @@ class Model(C.Structure):
                 ("T0", C.c_double), ("T_index", C.c_double), ("h_over_r", C.c_double), ("beta", C.c_double),
                 ("r_rt_out", C.c_double), ("tau_max", C.c_double), ("j_scale", C.c_double),
                 ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double),
-                ("rt_scheme", C.c_int32), ("precision", C.c_int32)]
+                ("rt_scheme", C.c_int32), ("precision", C.c_int32),
+                ("spot_r_orbit", C.c_double), ("spot_size", C.c_double), ("spot_phi0", C.c_double)]
 
 
 def _struct(cls, d):
@@ -88,7 +90,11 @@ def load_library():
     L.odyssey_last_error.restype = C.c_char_p
     L.odyssey_shutdown.restype = None
     L.odyssey_eval_math.argtypes = [C.c_int, C.c_int, dp, dp, dp, vp]
-    for name in EXPORTED_SYMBOLS[:9]:
+    L.odyssey_render_hotspot.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.POINTER(C.c_double), C.c_int,
+                                         dp, dp, dp, dp, dp, dp, dp, ip, ip, vp]
+    L.odyssey_render_hotspot_host.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.POINTER(C.c_double), C.c_int,
+                                              dp, dp, dp, dp, dp, dp, dp, ip, ip]
+    for name in EXPORTED_SYMBOLS[:11]:
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -181,6 +187,43 @@ def render_spectrum(scene, model, nu_hz):
     _check(L.odyssey_render_spectrum(C.byref(_struct(Scene, scene)), C.byref(_struct(Model, model)), nu, C.c_int(nf),
                                      _ptr(out["images"]), _ptr(out["nuLnu"]), _ptr(out["flag"]),
                                      _ptr(out["n_attempt"]), _stream(torch)))
+    return out
+
+
+def render_hotspot(scene, model, t_obs):
+    """odyssey_render_hotspot: images [nt, ny, nx], lightcurve [nt], spectrogram [nt, nbins] or None, and per
+    pixel g, r_e, phi_e, t_e, flag, n_attempt."""
+    torch = _torch()
+    L = load_library()
+    ny, nx, nt = scene["ny"], scene["nx"], len(t_obs)
+    t = (C.c_double * nt)(*[float(v) for v in t_obs])
+    f64 = dict(dtype=torch.float64, device="cuda")
+    nb = int(model.get("nbins", 0))
+    out = dict(images=torch.empty((max(nt, 1), ny, nx), **f64), lightcurve=torch.empty((max(nt, 1),), **f64),
+               spectrogram=torch.empty((max(nt, 1), nb), **f64) if nb > 0 else None,
+               g=torch.empty((ny, nx), **f64), r_e=torch.empty((ny, nx), **f64), phi_e=torch.empty((ny, nx), **f64),
+               t_e=torch.empty((ny, nx), **f64), flag=torch.empty((ny, nx), dtype=torch.int32, device="cuda"),
+               n_attempt=torch.empty((ny, nx), dtype=torch.int32, device="cuda"))
+    _check(L.odyssey_render_hotspot(C.byref(_struct(Scene, scene)), C.byref(_struct(Model, model)), t, C.c_int(nt),
+                                    _ptr(out["images"]), _ptr(out["lightcurve"]), _ptr(out["spectrogram"]),
+                                    _ptr(out["g"]), _ptr(out["r_e"]), _ptr(out["phi_e"]), _ptr(out["t_e"]),
+                                    _ptr(out["flag"]), _ptr(out["n_attempt"]), _stream(torch)))
+    return out
+
+
+def render_hotspot_host(scene, model, t_obs):
+    L = load_library()
+    ny, nx, nt = scene["ny"], scene["nx"], len(t_obs)
+    t = (C.c_double * nt)(*[float(v) for v in t_obs])
+    nb = int(model.get("nbins", 0))
+    out = dict(images=np.empty((max(nt, 1), ny, nx)), lightcurve=np.empty(max(nt, 1)),
+               spectrogram=np.empty((max(nt, 1), nb)) if nb > 0 else None,
+               g=np.empty((ny, nx)), r_e=np.empty((ny, nx)), phi_e=np.empty((ny, nx)), t_e=np.empty((ny, nx)),
+               flag=np.empty((ny, nx), np.int32), n_attempt=np.empty((ny, nx), np.int32))
+    _check(L.odyssey_render_hotspot_host(C.byref(_struct(Scene, scene)), C.byref(_struct(Model, model)), t, C.c_int(nt),
+                                         _np_ptr(out["images"]), _np_ptr(out["lightcurve"]), _np_ptr(out["spectrogram"]),
+                                         _np_ptr(out["g"]), _np_ptr(out["r_e"]), _np_ptr(out["phi_e"]), _np_ptr(out["t_e"]),
+                                         _np_ptr(out["flag"]), _np_ptr(out["n_attempt"])))
     return out
 
 

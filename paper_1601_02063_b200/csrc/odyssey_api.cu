@@ -97,8 +97,13 @@ int check_scene(const odyssey_scene* S) {
 
 int check_model(const odyssey_model* M) {
     if (!M) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "model is NULL");
-    if (M->kind < ODYSSEY_KIND_NONE || M->kind > ODYSSEY_KIND_RIAF) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown model kind %d", M->kind);
-    if (M->kind == ODYSSEY_KIND_THIN_DISK) {
+    if (M->kind < ODYSSEY_KIND_NONE || M->kind > ODYSSEY_KIND_HOT_SPOT) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown model kind %d", M->kind);
+    if (M->kind == ODYSSEY_KIND_HOT_SPOT) {
+        if (!(M->spot_size > 0.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spot_size = %g must be > 0", M->spot_size);
+        if (M->spot_r_orbit > 0.0 && !(M->spot_r_orbit > 1.0 + std::sqrt(1.0)))
+            return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spot_r_orbit = %g must lie outside the horizon (or be <= 0 for r_isco)", M->spot_r_orbit);
+    }
+    if (M->kind == ODYSSEY_KIND_THIN_DISK || M->kind == ODYSSEY_KIND_HOT_SPOT) {
         if (M->nbins < 0 || M->nbins > 4096) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nbins = %d outside [0, 4096]", M->nbins);
         if (M->nbins > 0 && !(M->g_hi > M->g_lo)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "g_hi must exceed g_lo");
     }
@@ -142,7 +147,16 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
     P->kind = M ? M->kind : 0;
     P->nf = nf;
     if (!M) return;
-    if (M->kind == ODYSSEY_KIND_THIN_DISK) {
+    if (M->kind == ODYSSEY_KIND_HOT_SPOT) {
+        const double rs = (M->spot_r_orbit > 0.0) ? M->spot_r_orbit : P->r_isco;
+        P->spot_R = std::sqrt(rs * rs + S.a * S.a);
+        P->spot_Omega = 1.0 / (rs * std::sqrt(rs) + S.a);
+        P->spot_phi0 = M->spot_phi0;
+        P->spot_inv2s2 = 1.0 / (2.0 * M->spot_size * M->spot_size);
+        P->spot_cut2 = 16.0 * M->spot_size * M->spot_size;
+        for (int k = 0; k < nf && k < MAX_FREQ; ++k) P->nu[k] = nu[k];          // the observer times t_obs[k]
+    }
+    if (M->kind == ODYSSEY_KIND_THIN_DISK || M->kind == ODYSSEY_KIND_HOT_SPOT) {
         P->r_in = (M->r_in > 0.0) ? M->r_in : P->r_isco;
         P->r_out = M->r_out; P->emis_index = M->emis_index; P->g_power = M->g_power;
         P->g_lo = M->g_lo; P->g_hi = M->g_hi; P->nbins = M->nbins;
@@ -172,6 +186,8 @@ constexpr int NT_SPEC = 128, MINB_SPEC = 3;     // 168 registers (the unrolled f
 typedef void (*KernelFn)(const Params, const Outputs);
 
 KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0, int prec = 0, bool time = false) {
+    if (kind == 3)
+        return tab ? odyssey_kernel<3, 1, false, NT_MAIN, MINB_MAIN, 0, 0, 1> : odyssey_kernel<3, 0, false, NT_MAIN, MINB_MAIN, 0, 0, 1>;
     if (kind == 0 && time)
         return tab ? odyssey_kernel<0, 1, false, NT_MAIN, MINB_MAIN, 0, 0, 1> : odyssey_kernel<0, 0, false, NT_MAIN, MINB_MAIN, 0, 0, 1>;
     if (kind == 2 && !spec && rts == 0 && prec == 1)
@@ -353,7 +369,7 @@ int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st) 
 // ---- host-buffer variants: device scratch, same kernels, copies back, synchronous -------------
 namespace {
 struct Scratch {
-    void* dev[12]; void* host[12]; size_t bytes[12]; int n = 0;
+    void* dev[16]; void* host[16]; size_t bytes[16]; int n = 0;
     ~Scratch() { for (int i = 0; i < n; ++i) if (dev[i]) cudaFreeAsync(dev[i], 0); }
     template <class T> int add(T* host_ptr, size_t count, T** out) {
         *out = nullptr;
@@ -428,6 +444,29 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
     return launch(P, O, true, scene->tableau, (cudaStream_t)cuda_stream);
 }
 
+int odyssey_render_hotspot(const odyssey_scene* scene, const odyssey_model* model, const double* t_obs_host, int nt,
+                           double* images, double* lightcurve, double* spectrogram,
+                           double* g, double* r_e, double* phi_e, double* t_e, int32_t* flag, int32_t* n_attempt,
+                           void* cuda_stream) {
+    int rc = check_scene(scene);
+    if (rc) return rc;
+    rc = check_model(model);
+    if (rc) return rc;
+    if (model->kind != ODYSSEY_KIND_HOT_SPOT) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "hot-spot mode needs model kind 3, got %d", model->kind);
+    if (nt < 1 || nt > ODYSSEY_MAX_FREQ) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nt = %d outside [1, %d]", nt, ODYSSEY_MAX_FREQ);
+    if (!t_obs_host) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "t_obs_host is NULL");
+    for (int k = 0; k < nt; ++k)
+        if (!std::isfinite(t_obs_host[k])) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "t_obs_host[%d] is not finite", k);
+    Params P; fill_params(*scene, model, t_obs_host, nt, &P);
+    Outputs O = no_outputs();
+    O.images = images; O.nuLnu = lightcurve; O.aux0 = g; O.aux1 = r_e; O.ph = phi_e; O.t = t_e;
+    O.flag = flag; O.n_attempt = n_attempt;
+    const bool spec = spectrogram && model->nbins > 0;
+    O.hist = spec ? spectrogram : nullptr;
+    if (spec) CUDA_TRY(cudaMemsetAsync(spectrogram, 0, sizeof(double) * (size_t)nt * model->nbins, (cudaStream_t)cuda_stream));
+    return launch(P, O, false, scene->tableau, (cudaStream_t)cuda_stream);
+}
+
 // ---- host-buffer variants (Scratch defined above) ---------------------------------------------
 
 int odyssey_trace_geodesics_host(const odyssey_scene* scene, int32_t* flag, double* r, double* theta, double* phi, double* t,
@@ -466,6 +505,21 @@ int odyssey_render_spectrum_host(const odyssey_scene* scene, const odyssey_model
     return S.copy_back();
 }
 
+int odyssey_render_hotspot_host(const odyssey_scene* scene, const odyssey_model* model, const double* t_obs_host, int nt,
+                                double* images, double* lightcurve, double* spectrogram,
+                                double* g, double* r_e, double* phi_e, double* t_e, int32_t* flag, int32_t* n_attempt) {
+    TRY(check_scene(scene)); TRY(check_model(model));
+    if (nt < 1 || nt > ODYSSEY_MAX_FREQ) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nt = %d outside [1, %d]", nt, ODYSSEY_MAX_FREQ);
+    const size_t n = (size_t)scene->nx * scene->ny;
+    Scratch S; double *dimg, *dlc, *dsp, *dg, *dre, *dph, *dte; int32_t *dflag, *datt;
+    TRY(S.add(images, n * nt, &dimg)); TRY(S.add(lightcurve, (size_t)nt, &dlc));
+    TRY(S.add(model->nbins > 0 ? spectrogram : nullptr, (size_t)nt * (size_t)(model->nbins > 0 ? model->nbins : 0), &dsp));
+    TRY(S.add(g, n, &dg)); TRY(S.add(r_e, n, &dre)); TRY(S.add(phi_e, n, &dph)); TRY(S.add(t_e, n, &dte));
+    TRY(S.add(flag, n, &dflag)); TRY(S.add(n_attempt, n, &datt));
+    TRY(odyssey_render_hotspot(scene, model, t_obs_host, nt, dimg, dlc, dsp, dg, dre, dph, dte, dflag, datt, nullptr));
+    return S.copy_back();
+}
+
 // ---- probes and bookkeeping ---------------------------------------------------------------------
 int odyssey_fp64_peak_probe(int iters, double* sink, double* flop_host, void* cuda_stream) {
     if (iters <= 0 || !sink) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "iters must be > 0 and sink non-NULL");
@@ -493,7 +547,7 @@ int odyssey_eval_math(int op, int n, const double* x, double* y, double* y2, voi
 
 int odyssey_kernel_info(int kind, int spectrum, int tableau, int32_t* regs, int32_t* local_bytes,
                         int32_t* threads_per_block, int32_t* blocks_per_sm, int32_t* n_sm) {
-    if (kind < 0 || kind > 2 || (tableau != 0 && tableau != 1)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown kind/tableau");
+    if (kind < 0 || kind > 3 || (tableau != 0 && tableau != 1)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown kind/tableau");
     DevState* D = nullptr;
     TRY(device_state(&D, nullptr));
     const bool spec = spectrum != 0;

@@ -237,7 +237,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         if (done && !fresh) {
             if (mode == M_NORMAL) {                                    // fresh accepted step: detect events
                 int m = M_NORMAL;
-                if (KIND == 1) {
+                if (KIND == 1 || KIND == 3) {
                     if (!on_eq && cos_y * cn < 0.0) m = M_EQ;          // equatorial crossing (reading P)
                     else on_eq = false;
                 }
@@ -345,6 +345,37 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                 if (O.image) O.image[pix] = 0.0;
                 if (O.aux0) O.aux0[pix] = 0.0;
                 if (O.aux1) O.aux1[pix] = 0.0;
+            } else if (KIND == 3) {
+                // hot spot on the equatorial plane (reading HS): brightness of the crossing point at each observer
+                // time t_obs[k] (kept in P.nu[k]), spot centre at the emission time t_obs + t_e (t_e = y_t < 0)
+                const bool hit = (flag == F_DISK && g_disk > 0.0);
+                if (O.aux0) O.aux0[pix] = g_disk;
+                if (O.aux1) O.aux1[pix] = r_e;
+                if (O.ph) O.ph[pix] = (flag == F_DISK) ? y.ph : 0.0;
+                if (O.t) O.t[pix] = (flag == F_DISK) ? y_t : 0.0;
+                const size_t npix = (size_t)P.nx * P.ny;
+                const double Re = sqrt(fma(r_e, r_e, P.a2));
+                const double gp = hit ? pow(g_disk, P.g_power) : 0.0;
+                // only crossings within 4 r_spot of the orbit can ever be lit
+                const bool near = hit && fabs(Re - P.spot_R) * fabs(Re - P.spot_R) < P.spot_cut2;
+                int b = -1;
+                if (hit && O.hist && P.nbins > 0 && g_disk >= P.g_lo && g_disk < P.g_hi) {
+                    b = (int)floor((g_disk - P.g_lo) / (P.g_hi - P.g_lo) * P.nbins);
+                    if (b >= P.nbins) b = P.nbins - 1;
+                }
+                for (int k = 0; k < P.nf; ++k) {
+                    double v = 0.0;
+                    if (near) {
+                        const double phis = fma(P.spot_Omega, P.nu[k] + y_t, P.spot_phi0);
+                        const double d2 = fma(Re, Re, P.spot_R * P.spot_R) - 2.0 * Re * P.spot_R * cos(y.ph - phis);
+                        if (d2 < P.spot_cut2) v = gp * exp(-d2 * P.spot_inv2s2);
+                    }
+                    if (O.images) O.images[(size_t)k * npix + pix] = v;
+                    if (v != 0.0) {
+                        if (O.nuLnu) atomicAdd(&O.nuLnu[k], v * P.pix_area);
+                        if (b >= 0) atomicAdd(&O.hist[(size_t)k * P.nbins + b], v * P.pix_area);
+                    }
+                }
             } else if (KIND == 1) {
                 double val = 0.0;
                 if (flag == F_DISK && g_disk > 0.0) val = pow(g_disk, P.g_power) * pow(r_e, -P.emis_index);

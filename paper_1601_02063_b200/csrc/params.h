@@ -40,6 +40,9 @@ struct Params {
     double sed_coef;                            // 4π r_g^2 Δx Δy
     int32_t nf, rt_scheme;                      // rt_scheme: ODYSSEY_RT_* (kind 2)
     int32_t precision, pad3;                    // ODYSSEY_PREC_* (kind 2)
+    // ---- hot spot (kind 3; eq. (36)); the observer times t_obs[k] travel in nu[k], nf = their number
+    double spot_R, spot_Omega, spot_phi0;       // sqrt(r_s² + a²), 1/(r_s^{3/2} + a), azimuth at t = 0
+    double spot_inv2s2, spot_cut2;              // 1/(2 r_spot²), (4 r_spot)²
     double nu[MAX_FREQ];
     double ln_nu[MAX_FREQ];
     double nu12[MAX_FREQ], inu12[MAX_FREQ];     // ν^(1/12) and its reciprocal (eq. (38) in powers of x_M^(1/12))

@@ -32,7 +32,7 @@ def test_header_symbols_are_all_exported():
 def test_struct_layout_matches_header_sizes():
     # 8 doubles + 2 int32 + double + 2 int32 + 3 doubles + 2 int32 = 15*8 = 120 bytes; model: 2 int32 + 16 doubles
     assert C.sizeof(B.Scene) == 120
-    assert C.sizeof(B.Model) == 8 + 16 * 8 + 8
+    assert C.sizeof(B.Model) == 8 + 16 * 8 + 8 + 3 * 8
 
 
 @pytest.mark.parametrize("patch, msg", [

@@ -279,3 +279,43 @@ def test_mixed_fp32_transfer_variant_accuracy_against_the_oracle(ody, orc, nu):
     a, b = _np(out["image"]).ravel(), _np(base["image"]).ravel()
     l1 = np.abs(a - b).sum() / b.sum()
     assert 1e-10 < l1 < 1e-6
+
+
+# ----------------------------------------------------------------------------- hot spot (kind 3, reading HS)
+@pytest.mark.parametrize("a, incl, n, hw, kw", [
+    (0.0, 60.0, 96, 10.0, dict()),                                   # the paper's set-up: Schwarzschild, i = 60 deg, r_spot 0.5 at r_isco
+    (0.9, 75.0, 80, 9.0, dict(r_spot=0.4)),
+    (0.5, 30.0, 64, 12.0, dict(r_orbit=8.0, r_spot=1.2, phi0=1.0, g_power=3.0, nbins=40)),
+])
+def test_hot_spot_matches_the_oracle(ody, orc, a, incl, n, hw, kw):
+    sc = W.scene(a, incl, n, hw)
+    mo = W.model_hot_spot(**kw)
+    rs = kw.get("r_orbit", 0.0) or orc.kerr_constants(a)["r_isco"]
+    period = 2.0 * np.pi * (rs ** 1.5 + a)
+    t_obs = list(np.linspace(0.0, period, 13)[:-1]) + [3.7 * period]
+    out = ody.render_hotspot(sc, mo, t_obs); _sync()
+    ref = orc.render_hotspot(sc, mo, t_obs)
+    gpu = {k: (_np(v) if v is not None else None) for k, v in out.items()}
+    assert np.array_equal(gpu["flag"].ravel(), ref["flag"])
+    hit = ref["flag"] == W.FLAG_DISK
+    for key in ("g", "r_e", "phi_e", "t_e"):
+        x, xr = gpu[key].ravel(), ref[key]
+        assert np.max(np.abs(x[hit] - xr[hit]) / np.abs(xr[hit])) <= 1e-8, key
+        assert np.all(x[~hit] == 0.0), key
+    imgs = gpu["images"].reshape(len(t_obs), -1)
+    lit = 0
+    for k in range(len(t_obs)):
+        if ref["images"][k].max() > 0:
+            lit += 1
+            # the Gaussian turns a 1e-8 relative error of phi_e, t_e into ~1e-7 of the value far out in its wings
+            assert np.abs(imgs[k] - ref["images"][k]).sum() / ref["images"][k].sum() <= 1e-6
+            on = ref["images"][k] >= 1e-6 * ref["images"][k].max()
+            assert np.max(np.abs(imgs[k] - ref["images"][k])[on] / ref["images"][k][on]) <= 1e-4
+    assert lit >= 6
+    assert np.allclose(gpu["lightcurve"], ref["lightcurve"], rtol=1e-6, atol=1e-12 * ref["lightcurve"].max())
+    assert np.allclose(gpu["spectrogram"].sum(axis=1), gpu["lightcurve"], rtol=1e-10, atol=1e-300)
+    assert np.max(np.abs(np.cumsum(gpu["spectrogram"], axis=1) - np.cumsum(ref["spectrogram"], axis=1))) <= 1e-6 * ref["lightcurve"].max()
+    # host entry point: same numbers
+    host = ody.render_hotspot_host(sc, mo, t_obs)
+    assert np.array_equal(host["images"], gpu["images"]) and np.array_equal(host["t_e"], gpu["t_e"])
+    assert np.allclose(host["lightcurve"], gpu["lightcurve"], rtol=1e-12)
