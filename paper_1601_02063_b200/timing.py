@@ -23,6 +23,8 @@ def time_case(ody, torch, name, w, reps):
     sc, mo, nu = w["scene"], w["model"], w["nu"]
 
     def call():
+        if mo["kind"] == W.KIND_HOT_SPOT:
+            return ody.render_hotspot(sc, mo, nu)
         if mo["kind"] == W.KIND_NONE:
             return ody.trace_geodesics(sc)
         if len(nu) > 1:
@@ -56,6 +58,8 @@ def main():
     import paper_1601_02063_b200 as ody
     cases = [("C0", W.C0()), ("C1", W.C1()), ("C2", W.C2()), ("C3", W.C3()), ("C4", W.C4())]
     cases.append(("C2 rt_scheme=RK components", dict(W.C2(), model=W.model_riaf(rt_scheme=W.RT_RK_COMPONENTS))))
+    t_obs = [2.0 * 3.141592653589793 * 6.0 ** 1.5 * k / 32 for k in range(32)]
+    cases.append(("hot spot a=0 i=60 512^2, 32 phases", dict(scene=W.scene(0.0, 60.0, 512, 10.0), model=W.model_hot_spot(), nu=t_obs)))
     if args.sweep:
         for a in (0.0, 0.5, 0.9, 0.998):
             for n in (1024, 2048, 4096):

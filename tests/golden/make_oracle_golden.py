@@ -33,6 +33,12 @@ def main():
     w = W.C3(n=4, nf=4)
     s = O.render_spectrum(w["scene"], w["model"], w["nu"])
     out["C3_4x4_nf4"] = {"nu": list(w["nu"]), "nuLnu": s["nuLnu"].tolist(), "images": s["images"].tolist()}
+    sc = W.scene(0.5, 60.0, 10, 9.0)
+    hs = O.render_hotspot(sc, W.model_hot_spot(r_spot=1.0, nbins=8), [0.0, 40.0, 80.0])
+    out["hotspot_10x10"] = {"t_obs": [0.0, 40.0, 80.0], "lightcurve": hs["lightcurve"].tolist(), "t_e": hs["t_e"].tolist(),
+                            "phi_e": hs["phi_e"].tolist(), "images": hs["images"].tolist()}
+    g = O.trace_geodesics(W.C0(n=8)["scene"])
+    out["C0_8x8"]["t"] = g["t"].tolist()
     with open(os.path.join(HERE, "oracle_regression.json"), "w") as f:
         json.dump(out, f, indent=1)
     print("wrote oracle_regression.json")

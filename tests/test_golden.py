@@ -82,6 +82,10 @@ def test_oracle_regression_values():
     assert g["flag"].tolist() == ref["flag"] and g["n_attempt"].tolist() == ref["n_attempt"]
     for k in ("r", "th", "ph"):
         _cmp(g[k], ref[k], 1e-12)
+    _cmp(g["t"], ref["t"], 1e-12)
+    hs = O.render_hotspot(W.scene(0.5, 60.0, 10, 9.0), W.model_hot_spot(r_spot=1.0, nbins=8), ORACLE["hotspot_10x10"]["t_obs"])
+    _cmp(hs["lightcurve"], ORACLE["hotspot_10x10"]["lightcurve"], 1e-10)
+    _cmp(hs["t_e"], ORACLE["hotspot_10x10"]["t_e"], 1e-12)
     w = W.C1(n=8)
     d = O.render_image(w["scene"], w["model"])
     assert d["flag"].tolist() == ORACLE["C1_8x8"]["flag"]
@@ -103,6 +107,11 @@ def test_cuda_path_against_stored_oracle_values(ody):
     assert out["flag"].cpu().numpy().ravel().tolist() == ref["flag"]
     _cmp(out["theta"].cpu().numpy(), ref["th"], 1e-8)
     _cmp(out["phi"].cpu().numpy(), ref["ph"], 1e-8)
+    hs = ody.render_hotspot(W.scene(0.5, 60.0, 10, 9.0), W.model_hot_spot(r_spot=1.0, nbins=8), ORACLE["hotspot_10x10"]["t_obs"])
+    torch.cuda.synchronize()
+    _cmp(hs["lightcurve"].cpu().numpy(), ORACLE["hotspot_10x10"]["lightcurve"], 1e-6)
+    tt = ody.trace_geodesics(W.C0(n=8)["scene"], with_time=True); torch.cuda.synchronize()
+    _cmp(tt["t"].cpu().numpy(), ref["t"], 1e-8)
     w = W.C2(n=8)
     for scheme in (W.RT_PER_STEP, W.RT_RK_COMPONENTS):
         r = ody.render_image(w["scene"], dict(w["model"], rt_scheme=scheme), w["nu"][0]); torch.cuda.synchronize()
