@@ -411,6 +411,7 @@ int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model,
     if (rc) return rc;
     rc = check_model(model);
     if (rc) return rc;
+    if (model->kind == ODYSSEY_KIND_HOT_SPOT) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "model kind 3 (hot spot) is rendered by odyssey_render_hotspot");
     if (model->kind == ODYSSEY_KIND_RIAF && !(nu_hz > 0.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz = %g must be > 0", nu_hz);
     Params P; fill_params(*scene, model, &nu_hz, 1, &P);
     Outputs O = no_outputs();

@@ -71,6 +71,15 @@ def test_invalid_model_and_frequencies_are_rejected():
     mixed = B._struct(B.Model, w["model"]); mixed.precision = 1
     assert L.odyssey_render_spectrum(C.byref(sc), C.byref(mixed), nu, 4, None, None, None, None, None) == -1
     assert "precision" in ody.last_error()
+    spot = B._struct(B.Model, W.model_hot_spot())
+    assert L.odyssey_render_image(C.byref(sc), C.byref(spot), C.c_double(1e9),
+                                  None, None, None, None, None, None, None, None) == -1
+    assert "odyssey_render_hotspot" in ody.last_error()
+    tt = (C.c_double * 40)(*([0.0] * 40))
+    assert L.odyssey_render_hotspot(C.byref(sc), C.byref(spot), tt, 33, *([None] * 10)) == -1
+    assert L.odyssey_render_hotspot(C.byref(sc), C.byref(mo), tt, 4, *([None] * 10)) == -1      # RIAF model in hot-spot mode
+    bad_spot = B._struct(B.Model, W.model_hot_spot(r_spot=0.0))
+    assert L.odyssey_render_hotspot(C.byref(sc), C.byref(bad_spot), tt, 4, *([None] * 10)) == -1
     thin = B._struct(B.Model, W.C1()["model"])
     assert L.odyssey_render_spectrum(C.byref(sc), C.byref(thin), nu, 4, None, None, None, None, None) == -1
     assert L.odyssey_render_image(None, None, C.c_double(0.0), None, None, None, None, None, None, None, None) == -1
