@@ -25,8 +25,12 @@
  *   - Return value: ODYSSEY_OK (0) or a negative odyssey_status.  After a failure
  *     odyssey_last_error() returns a static, thread-local, NUL-terminated description.
  *     Nothing is printed, nothing throws.
- *   - The library owns only a small ring of work-queue counters per device (allocated lazily,
- *     released by odyssey_shutdown()).
+ *   - The library owns a small ring of 64 work-queue counters per device (allocated lazily, released
+ *     by odyssey_shutdown(); every launch takes the next one, so up to 64 launches may be in flight at
+ *     once) and takes its scratch (initial states: 48 bytes per pixel; spectrum mode: see there) from
+ *     the device's default stream-ordered memory pool (cudaMallocAsync / cudaFreeAsync on `cuda_stream`).
+ *   - Every call first runs a camera kernel (initial conditions of all pixels), then the persistent
+ *     integrator kernel: two kernel launches of this library per call (more in spectrum mode).
  */
 #ifndef ODYSSEY_H_
 #define ODYSSEY_H_
@@ -48,7 +52,7 @@ typedef enum odyssey_status {
 enum {
     ODYSSEY_FLAG_ESCAPED = 0,  /* p_r > 0 and r >= r_esc; final state located ON r = r_esc          */
     ODYSSEY_FLAG_CAPTURED = 1, /* r <= r_h + horizon_eps; final state located ON that radius         */
-    ODYSSEY_FLAG_DISK = 2,     /* kind 1: first equatorial crossing with r_in <= r <= r_out           */
+    ODYSSEY_FLAG_DISK = 2,     /* kinds 1, 3: first equatorial crossing with r_in <= r <= r_out       */
     ODYSSEY_FLAG_OPAQUE = 3,   /* kind 2: every frequency has tau > tau_max                           */
     ODYSSEY_FLAG_MAXSTEP = 4   /* max_attempts Runge–Kutta attempts used                              */
 };
