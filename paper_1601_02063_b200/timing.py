@@ -60,6 +60,9 @@ def main():
     cases.append(("C2 rt_scheme=RK components", dict(W.C2(), model=W.model_riaf(rt_scheme=W.RT_RK_COMPONENTS))))
     t_obs = [2.0 * 3.141592653589793 * 6.0 ** 1.5 * k / 32 for k in range(32)]
     cases.append(("hot spot a=0 i=60 512^2, 32 phases", dict(scene=W.scene(0.0, 60.0, 512, 10.0), model=W.model_hot_spot(), nu=t_obs)))
+    # the set-up of the paper's own timing table (Table 1: geodesics only, a = 0.95, i = 60 deg,
+    # 1024^2; the image-plane extent is not stated there: +/-10 M is used)
+    cases.append(("paper Table 1 set-up: geodesics only a=0.95 i=60 1024^2", dict(scene=W.scene(0.95, 60.0, 1024, 10.0), model=W.model_none(), nu=[])))
     if args.sweep:
         for a in (0.0, 0.5, 0.9, 0.998):
             for n in (1024, 2048, 4096):
