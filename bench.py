@@ -384,7 +384,7 @@ def run_b200(args):
                        "ms_per_step": e2e_s_max / args.steps * 1e3,
                        "api": "odyssey_render_image_host (pinned host buffers; device scratch, kernel and D2H copies "
                               "of all six output arrays inside the timed region)"}
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and world == 1:                       # the oracle leg runs at N = 1 only
         from oracle import build as oracle_build
         oracle_build.build()
         line["cpu_baseline"] = cpu_baseline(w, args.cpu_sample)
