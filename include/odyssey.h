@@ -58,7 +58,7 @@ enum {
 };
 
 enum { ODYSSEY_TABLEAU_RKF45 = 0, ODYSSEY_TABLEAU_CASH_KARP = 1 };
-enum { ODYSSEY_KIND_NONE = 0, ODYSSEY_KIND_THIN_DISK = 1, ODYSSEY_KIND_RIAF = 2, ODYSSEY_KIND_HOT_SPOT = 3 };
+enum { ODYSSEY_KIND_NONE = 0, ODYSSEY_KIND_THIN_DISK = 1, ODYSSEY_KIND_RIAF = 2, ODYSSEY_KIND_HOT_SPOT = 3, ODYSSEY_KIND_NT_DISK = 4 };
 /* PAPER.md:L171 says the transfer equations are "easily integrated along with the geodesic … piecewise
  * according to these steps".  PER_STEP (default): one update per accepted step, trapezoid in lambda with
  * the exact attenuation across the step.  RK_COMPONENTS: tau and I as two more components of the
@@ -107,6 +107,7 @@ typedef struct odyssey_model {
     double spot_r_orbit;       /* kind 3: radius of the spot's circular equatorial orbit; <= 0 means r_isco(a)  */
     double spot_size;          /* kind 3: r_spot of eq. (36) (the paper uses 0.5 r_g); emission is cut at 4 r_spot */
     double spot_phi0;          /* kind 3: azimuth of the spot centre at coordinate time t = 0                    */
+    double mdot_gs;            /* kind 4: accretion rate in g/s (eq. (35)); uses mbh_msun, r_in (<= 0: r_isco), r_out */
 } odyssey_model;
 
 /* Geodesics only (BASELINE.json:configs[0]; §2.1-2.2).  Per pixel: outcome flag, the
@@ -124,6 +125,8 @@ int odyssey_trace_geodesics(const odyssey_scene* scene,
  *     (hist is overwritten, not accumulated across calls).
  *   kind 2 (eqs. (30),(31),(37)-(39)): image = I_nu = nu^3 × invariant intensity (erg s^-1 cm^-2
  *     Hz^-1 sr^-1), aux0 = optical depth tau, aux1 = 0.
+ *   kind 4 (eq. (35)): image = I_nu of the Novikov–Thorne disk at nu_hz (see
+ *     odyssey_render_spectrum), aux0 = g, aux1 = r_e as for kind 1.
  *   kind 0: image = aux0 = aux1 = 0; flags and step counts as odyssey_trace_geodesics.
  * n_attempt / n_accept: attempted and accepted Runge–Kutta steps per ray (one radiative-transfer
  * update is made per accepted step).                                               */
@@ -136,7 +139,14 @@ int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model,
  * (erg/s; the distance cancels).  nu_hz_host is HOST memory.  rt_scheme must be ODYSSEY_RT_PER_STEP.
  * Images with fewer rays than four waves of resident lanes (~3e5 pixels on a B200) take a two-phase path
  * (record the geodesics once, then one lane per (ray, frequency)); that path synchronises `cuda_stream`
- * ONCE inside the call to read an overflow flag, and uses stream-ordered scratch (up to 28 KB per ray).   */
+ * ONCE inside the call to read an overflow flag, and uses stream-ordered scratch (up to 28 KB per ray).
+ *
+ * kind 4, the relativistic multi-temperature disk of Novikov & Thorne (eq. (35), Fig. 6): an
+ * opaque disk on the equatorial plane between r_in (<= 0: r_isco) and r_out whose surface radiates as a blackbody
+ * at T_eff(r), sigma T_eff^4 = 3 Mdot M f(r) / (8 pi r^3) in G = c = 1, f = Page & Thorne's zero-torque function
+ * (0 at and inside r_isco).  One geodesic pass; at the first crossing, for every frequency,
+ * images[k] = I_nu = (2 h nu^3 / c^2) / expm1(h nu / (g k_B T_eff(r_e))) (the invariance of I_nu / nu^3 with the
+ * redshift g of eq. (2)), and nuLnu[k] as above.  No stream synchronisation, no scratch beyond the camera pass. */
 int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* model,
                             const double* nu_hz_host, int nf,
                             double* images, double* nuLnu, int32_t* flag, int32_t* n_attempt,

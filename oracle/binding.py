@@ -32,7 +32,8 @@ class Model(C.Structure):
                 ("r_rt_out", C.c_double), ("tau_max", C.c_double), ("j_scale", C.c_double),
                 ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double),
                 ("rt_scheme", C.c_int32), ("pad", C.c_int32),
-                ("spot_r_orbit", C.c_double), ("spot_size", C.c_double), ("spot_phi0", C.c_double)]
+                ("spot_r_orbit", C.c_double), ("spot_size", C.c_double), ("spot_phi0", C.c_double),
+                ("mdot_gs", C.c_double)]
 
 
 def _fill(struct, d):
@@ -179,6 +180,16 @@ def rt_update(a0, a1, e0, e1, dl, tau_max, tau, T, I):
     lib().oracle_rt_update(C.c_double(a0), C.c_double(a1), C.c_double(e0), C.c_double(e1), C.c_double(dl),
                            C.c_double(tau_max), _dp(st))
     return st[0], st[1], st[2]
+
+
+def page_thorne_f(a, r):
+    L = lib(); L.oracle_page_thorne_f.restype = C.c_double
+    return L.oracle_page_thorne_f(C.c_double(a), C.c_double(r))
+
+
+def nt_temperature(model, a, r):
+    L = lib(); L.oracle_nt_temperature.restype = C.c_double
+    return L.oracle_nt_temperature(C.byref(make_model(model)), C.c_double(a), C.c_double(r))
 
 
 def rt_rk_step(which, a, eps, h, tau_max, tau, I):

@@ -56,6 +56,8 @@ constexpr double M_ELECTRON = 9.1093837015e-28;  // g
 constexpr double M_PROTON = 1.67262192369e-24;   // g
 constexpr double E_CHARGE = 4.80320471257e-10;   // esu
 constexpr double PI = 3.14159265358979323846;
+constexpr double G_NEWTON = 6.67430e-8;          // cm^3 g^-1 s^-2
+constexpr double SIGMA_SB = 5.670374419e-5;      // erg cm^-2 s^-1 K^-4
 
 enum Flag { ESCAPED = 0, CAPTURED = 1, DISK = 2, OPAQUE = 3, MAXSTEP = 4 };
 
@@ -76,6 +78,7 @@ struct Model {           // mirrors workloads.model_*()
     double g_lo, g_hi, g_power;
     int32_t rt_scheme, pad;  // 0: one update per accepted step [reading E]; 1: tau, I as Runge-Kutta components [E']
     double spot_r_orbit, spot_size, spot_phi0;   // kind 3 [reading HS]: orbit radius (<= 0: r_isco), r_spot, azimuth at t = 0
+    double mdot_gs;                              // kind 4 [reading NT]: accretion rate, g/s
 };
 
 // ----------------------------------------------------------------------------------------------
@@ -474,7 +477,7 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
         };
 
         // (1) thin disk: equatorial crossing inside the step [reading P]
-        if ((M.kind == 1 || M.kind == 3) && !on_equator && std::cos(y[1]) * std::cos(ynew[1]) < 0.0) {
+        if ((M.kind == 1 || M.kind == 3 || M.kind == 4) && !on_equator && std::cos(y[1]) * std::cos(ynew[1]) < 0.0) {
             locate(1, 0.5 * PI);
             on_equator = true;
             if (ynew[0] >= r_in && ynew[0] <= M.r_out && ynew[0] > r_cap) {
@@ -535,6 +538,44 @@ inline void pixel_xy(const Scene& S, int i, int j, double* x, double* y) {   // 
 double disk_value(const Model& M, const RayOut& R) {
     if (R.flag != DISK || !(R.g > 0.0)) return 0.0;
     return std::pow(R.g, M.g_power) * std::pow(R.r_e, -M.emis_index);
+}
+
+// Kind 4 [reading NT of PAPER.md:L225-238, eq. (35)]: the relativistic multi-temperature disk of Novikov & Thorne
+// (1973) / Page & Thorne (1974).  eq. (35): F(r) = 3 Mdot M f(r) / (8 pi r^3) = sigma T_eff^4; the paper does not
+// print f(r) ("a correction factor related to the inner boundary of the disk and relativistic effects" that vanishes
+// at r_isco).  It is Page & Thorne's closed form for zero torque at the marginally stable orbit, with x = sqrt(r),
+// x0 = sqrt(r_isco) and x1, x2, x3 the roots of x^3 - 3x + 2a = 0:
+//   f = x^2/(x^3 - 3x + 2a) [ x - x0 - (3/2) a ln(x/x0) - sum_i 3 (x_i - a)^2 / (x_i (x_i - x_j)(x_i - x_k)) ln((x - x_i)/(x0 - x_i)) ],
+// which tends to 1 - ... -> 1 far out (the Newtonian 3 G M Mdot / 8 pi r^3).
+double page_thorne_f(double a, double r) {
+    const double r0 = isco_radius(a);
+    if (!(r > r0)) return 0.0;
+    const double x = std::sqrt(r), x0 = std::sqrt(r0);
+    const double th = std::acos(a) / 3.0;
+    const double x1 = 2.0 * std::cos(th - PI / 3.0), x2 = 2.0 * std::cos(th + PI / 3.0), x3 = -2.0 * std::cos(th);
+    auto term = [&](double xi, double xj, double xk) {
+        return 3.0 * (xi - a) * (xi - a) / (xi * (xi - xj) * (xi - xk)) * std::log((x - xi) / (x0 - xi));
+    };
+    const double br = x - x0 - 1.5 * a * std::log(x / x0) - term(x1, x2, x3) - term(x2, x1, x3) - term(x3, x1, x2);
+    return x * x / (x * x * x - 3.0 * x + 2.0 * a) * br;
+}
+
+// T_eff(r) in kelvin from eq. (35) in cgs: F = 3 Mdot c^6 f / (8 pi G^2 M^2 r^3) with r in units of G M / c^2.
+double nt_temperature(const Model& M, double a, double r) {
+    const double Mg = GM_SUN * M.mbh_msun / G_NEWTON;                 // mass in grams
+    const double c6 = std::pow(C_LIGHT, 6);
+    const double F = 3.0 * M.mdot_gs * c6 * page_thorne_f(a, r) / (8.0 * PI * G_NEWTON * G_NEWTON * Mg * Mg * r * r * r);
+    return (F > 0.0) ? std::pow(F / SIGMA_SB, 0.25) : 0.0;
+}
+
+// Observed specific intensity of the disk surface (blackbody at T_eff, no colour correction): the invariant
+// I_nu / nu^3 is conserved, so I_nu(obs) = g^3 B_{nu/g}(T_eff(r_e)) = (2 h nu^3 / c^2) / expm1(h nu / (g k T_eff)).
+double nt_intensity(const Scene& S, const Model& M, const RayOut& R, double nu) {
+    if (R.flag != DISK || !(R.g > 0.0)) return 0.0;
+    const double T = nt_temperature(M, S.a, R.r_e);
+    if (!(T > 0.0)) return 0.0;
+    const double xx = H_PLANCK * nu / (R.g * K_BOLTZ * T);
+    return (2.0 * H_PLANCK * nu * nu * nu / (C_LIGHT * C_LIGHT)) / std::expm1(xx);
 }
 
 // Kind 3 [reading HS of PAPER.md:L252-264, eq. (36), Figs. 7, 8]: a hot spot on the opaque equatorial plane.
@@ -656,6 +697,9 @@ void oracle_synchrotron(const Model* M, double a, double r, double th, double nu
 void oracle_rt_update(double a0, double a1, double e0, double e1, double dl, double tau_max, double* state) {
     rt_update(a0, a1, e0, e1, dl, tau_max, &state[0], &state[1], &state[2]);
 }
+
+double oracle_page_thorne_f(double a, double r) { return page_thorne_f(a, r); }
+double oracle_nt_temperature(const Model* M, double a, double r) { return nt_temperature(*M, a, r); }
 
 // a[6], eps[6]: coefficients at the six stages; state = {tau, I}, updated in place [reading E']
 void oracle_rt_rk_step(int which, const double* a, const double* eps, double h, double tau_max, double* state) {
@@ -805,6 +849,13 @@ void oracle_render_spectrum(const Scene* S, const Model* M, const double* nu_hz,
         int i = idx_i ? idx_i[k] : k % S->nx, j = idx_j ? idx_j[k] : k / S->nx;
         double x, y; pixel_xy(*S, i, j, &x, &y);
         RayOut R;
+        if (M->kind == 4) {                      // Novikov-Thorne disk: evaluated at the crossing, no transfer along the ray
+            trace_ray(*S, *M, 0, nullptr, x, y, &R, nullptr);
+            for (int q = 0; q < nf; ++q) images[(size_t)q * n + k] = nt_intensity(*S, *M, R, nu_hz[q]);
+            if (flag) flag[k] = R.flag;
+            if (n_attempt) n_attempt[k] = R.n_attempt;
+            continue;
+        }
         trace_ray(*S, *M, nf, nu_hz, x, y, &R, nullptr);
         for (int q = 0; q < nf; ++q) images[(size_t)q * n + k] = nu_hz[q] * nu_hz[q] * nu_hz[q] * R.I[q];
         if (flag) flag[k] = R.flag;

@@ -45,7 +45,8 @@ class Model(C.Structure):
                 ("r_rt_out", C.c_double), ("tau_max", C.c_double), ("j_scale", C.c_double),
                 ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double),
                 ("rt_scheme", C.c_int32), ("precision", C.c_int32),
-                ("spot_r_orbit", C.c_double), ("spot_size", C.c_double), ("spot_phi0", C.c_double)]
+                ("spot_r_orbit", C.c_double), ("spot_size", C.c_double), ("spot_phi0", C.c_double),
+                ("mdot_gs", C.c_double)]
 
 
 def _struct(cls, d):

@@ -205,4 +205,20 @@ __device__ __forceinline__ void rt_update(const double a0, const double a1, cons
     tau = live ? tau + dtau : tau;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Novikov–Thorne disk (kind 4; eq. (35); reading NT): effective temperature at radius r,
+// σ T_eff⁴ = 3 Mdot M f(r)/(8π r³) with Page & Thorne's closed form of f for zero torque at r_isco,
+//   f = x²/(x³ - 3x + 2a) [x - x0 - (3/2) a ln(x/x0) - Σ_i c_i ln((x - x_i)/(x0 - x_i))],  x = sqrt(r).
+// Evaluated once per ray (at its disk crossing), so the library's log/pow are used as they are.
+__device__ __forceinline__ double nt_temperature(const Params& P, double r) {
+    if (!(r > P.r_isco)) return 0.0;
+    const double x = sqrt(r), x0 = P.nt_x0;
+    double br = x - x0 - 1.5 * P.a * log(x / x0);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) br -= P.nt_c[i] * log((x - P.nt_x[i]) / (x0 - P.nt_x[i]));
+    const double f = x * x / (x * x * x - 3.0 * x + 2.0 * P.a) * br;
+    const double T4 = P.nt_T4 * f / (r * r * r);
+    return (T4 > 0.0) ? sqrt(sqrt(T4)) : 0.0;
+}
+
 }  // namespace ody

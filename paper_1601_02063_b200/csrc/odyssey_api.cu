@@ -20,6 +20,7 @@ using namespace ody;
 constexpr double kC = 2.99792458e10, kGMsun = 1.3271244e26, kH = 6.62607015e-27, kKB = 1.380649e-16;
 constexpr double kMe = 9.1093837015e-28, kMp = 1.67262192369e-24, kE = 4.80320471257e-10;
 constexpr double kPi = 3.14159265358979323846;
+constexpr double kG = 6.67430e-8, kSigmaSB = 5.670374419e-5;
 
 thread_local char g_err[512] = "";
 std::atomic<long long> g_launches{0};
@@ -97,7 +98,7 @@ int check_scene(const odyssey_scene* S) {
 
 int check_model(const odyssey_model* M) {
     if (!M) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "model is NULL");
-    if (M->kind < ODYSSEY_KIND_NONE || M->kind > ODYSSEY_KIND_HOT_SPOT) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown model kind %d", M->kind);
+    if (M->kind < ODYSSEY_KIND_NONE || M->kind > ODYSSEY_KIND_NT_DISK) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown model kind %d", M->kind);
     if (M->kind == ODYSSEY_KIND_HOT_SPOT) {
         if (!(M->spot_size > 0.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spot_size = %g must be > 0", M->spot_size);
         if (M->spot_r_orbit > 0.0 && !(M->spot_r_orbit > 1.0 + std::sqrt(1.0)))
@@ -106,6 +107,10 @@ int check_model(const odyssey_model* M) {
     if (M->kind == ODYSSEY_KIND_THIN_DISK || M->kind == ODYSSEY_KIND_HOT_SPOT) {
         if (M->nbins < 0 || M->nbins > 4096) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nbins = %d outside [0, 4096]", M->nbins);
         if (M->nbins > 0 && !(M->g_hi > M->g_lo)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "g_hi must exceed g_lo");
+    }
+    if (M->kind == ODYSSEY_KIND_NT_DISK) {
+        if (!(M->mbh_msun > 0.0) || !(M->mdot_gs >= 0.0) || !(M->r_out > 0.0))
+            return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "Novikov-Thorne disk needs mbh_msun > 0, mdot_gs >= 0, r_out > 0");
     }
     if (M->kind == ODYSSEY_KIND_RIAF) {
         if (M->rt_scheme != ODYSSEY_RT_PER_STEP && M->rt_scheme != ODYSSEY_RT_RK_COMPONENTS)
@@ -156,6 +161,26 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
         P->spot_cut2 = 16.0 * M->spot_size * M->spot_size;
         for (int k = 0; k < nf && k < MAX_FREQ; ++k) P->nu[k] = nu[k];          // the observer times t_obs[k]
     }
+    if (M->kind == ODYSSEY_KIND_NT_DISK) {
+        // Page & Thorne's f(r) (emission.cuh: nt_temperature): roots of x³ - 3x + 2a and their weights
+        const double th = std::acos(S.a) / 3.0;
+        const double x[3] = {2.0 * std::cos(th - kPi / 3.0), 2.0 * std::cos(th + kPi / 3.0), -2.0 * std::cos(th)};
+        for (int i = 0; i < 3; ++i) {
+            const double xi = x[i], xj = x[(i + 1) % 3], xk = x[(i + 2) % 3];
+            P->nt_x[i] = xi;
+            P->nt_c[i] = 3.0 * (xi - S.a) * (xi - S.a) / (xi * (xi - xj) * (xi - xk));
+        }
+        P->nt_x0 = std::sqrt(P->r_isco);
+        const double Mg = kGMsun * M->mbh_msun / kG;                                   // grams
+        P->nt_T4 = 3.0 * M->mdot_gs * std::pow(kC, 6) / (8.0 * kPi * kG * kG * Mg * Mg * kSigmaSB);
+        P->h_over_k = kH / kKB;
+        P->planck2 = 2.0 * kH / (kC * kC);
+        P->r_in = (M->r_in > 0.0) ? M->r_in : P->r_isco;
+        P->r_out = M->r_out;
+        P->rg_cm = kGMsun * M->mbh_msun / (kC * kC);
+        P->sed_coef = 4.0 * kPi * P->rg_cm * P->rg_cm * P->pix_area;
+        for (int k = 0; k < nf && k < MAX_FREQ; ++k) { P->nu[k] = nu[k]; P->nu3[k] = nu[k] * nu[k] * nu[k]; }
+    }
     if (M->kind == ODYSSEY_KIND_THIN_DISK || M->kind == ODYSSEY_KIND_HOT_SPOT) {
         P->r_in = (M->r_in > 0.0) ? M->r_in : P->r_isco;
         P->r_out = M->r_out; P->emis_index = M->emis_index; P->g_power = M->g_power;
@@ -188,6 +213,8 @@ typedef void (*KernelFn)(const Params, const Outputs);
 KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0, int prec = 0, bool time = false) {
     if (kind == 3)
         return tab ? odyssey_kernel<3, 1, false, NT_MAIN, MINB_MAIN, 0, 0, 1> : odyssey_kernel<3, 0, false, NT_MAIN, MINB_MAIN, 0, 0, 1>;
+    if (kind == 4)
+        return tab ? odyssey_kernel<4, 1, false, NT_MAIN, MINB_MAIN> : odyssey_kernel<4, 0, false, NT_MAIN, MINB_MAIN>;
     if (kind == 0 && time)
         return tab ? odyssey_kernel<0, 1, false, NT_MAIN, MINB_MAIN, 0, 0, 1> : odyssey_kernel<0, 0, false, NT_MAIN, MINB_MAIN, 0, 0, 1>;
     if (kind == 2 && !spec && rts == 0 && prec == 1)
@@ -208,6 +235,7 @@ size_t smem_bytes(int kind, bool spec, int nf, int nbins, int rts = 0) {
     if (spec) return (size_t)(smem_per_thread(0) * NT_SPEC + MAX_FREQ) * sizeof(double);
     const size_t stages = (size_t)smem_per_thread(kind == 2 ? rts : 0) * NT_MAIN * sizeof(double);   // stage values + [5][NT] RT state
     if (kind == 1) return stages + (size_t)(nbins > 0 ? nbins : 1) * sizeof(double);
+    if (kind == 4) return stages + (size_t)MAX_FREQ * sizeof(double);
     return stages;
 }
 
@@ -412,9 +440,11 @@ int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model,
     rc = check_model(model);
     if (rc) return rc;
     if (model->kind == ODYSSEY_KIND_HOT_SPOT) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "model kind 3 (hot spot) is rendered by odyssey_render_hotspot");
-    if (model->kind == ODYSSEY_KIND_RIAF && !(nu_hz > 0.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz = %g must be > 0", nu_hz);
+    if ((model->kind == ODYSSEY_KIND_RIAF || model->kind == ODYSSEY_KIND_NT_DISK) && !(nu_hz > 0.0))
+        return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz = %g must be > 0", nu_hz);
     Params P; fill_params(*scene, model, &nu_hz, 1, &P);
     Outputs O = no_outputs();
+    if (model->kind == ODYSSEY_KIND_NT_DISK) O.images = image;      // the one-frequency case of the spectrum epilogue
     O.image = image; O.aux0 = aux0; O.aux1 = aux1; O.flag = flag; O.n_attempt = n_attempt; O.n_accept = n_accept;
     O.hist = (model->kind == ODYSSEY_KIND_THIN_DISK && model->nbins > 0) ? hist : nullptr;
     return launch(P, O, false, scene->tableau, (cudaStream_t)cuda_stream);
@@ -426,7 +456,18 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
     if (rc) return rc;
     rc = check_model(model);
     if (rc) return rc;
-    if (model->kind != ODYSSEY_KIND_RIAF) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode needs model kind 2 (RIAF), got %d", model->kind);
+    if (model->kind != ODYSSEY_KIND_RIAF && model->kind != ODYSSEY_KIND_NT_DISK)
+        return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode needs model kind 2 (RIAF) or 4 (Novikov-Thorne disk), got %d", model->kind);
+    if (model->kind == ODYSSEY_KIND_NT_DISK) {
+        if (nf < 1 || nf > ODYSSEY_MAX_FREQ) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nf = %d outside [1, %d]", nf, ODYSSEY_MAX_FREQ);
+        if (!nu_hz_host) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz_host is NULL");
+        for (int k = 0; k < nf; ++k)
+            if (!(nu_hz_host[k] > 0.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz_host[%d] = %g must be > 0", k, nu_hz_host[k]);
+        Params P; fill_params(*scene, model, nu_hz_host, nf, &P);
+        Outputs O = no_outputs();
+        O.images = images; O.nuLnu = nuLnu; O.flag = flag; O.n_attempt = n_attempt;
+        return launch(P, O, false, scene->tableau, (cudaStream_t)cuda_stream);      // one geodesic pass, all frequencies at the crossing
+    }
     if (model->rt_scheme != ODYSSEY_RT_PER_STEP) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode supports rt_scheme 0 (per-step update) only");
     if (model->precision != ODYSSEY_PREC_FP64) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode supports precision FP64 only");
     if (nf < 1 || nf > ODYSSEY_MAX_FREQ) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nf = %d outside [1, %d]", nf, ODYSSEY_MAX_FREQ);
@@ -548,7 +589,7 @@ int odyssey_eval_math(int op, int n, const double* x, double* y, double* y2, voi
 
 int odyssey_kernel_info(int kind, int spectrum, int tableau, int32_t* regs, int32_t* local_bytes,
                         int32_t* threads_per_block, int32_t* blocks_per_sm, int32_t* n_sm) {
-    if (kind < 0 || kind > 3 || (tableau != 0 && tableau != 1)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown kind/tableau");
+    if (kind < 0 || kind > 4 || (tableau != 0 && tableau != 1)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown kind/tableau");
     DevState* D = nullptr;
     TRY(device_state(&D, nullptr));
     const bool spec = spectrum != 0;

@@ -79,7 +79,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
 #define RT1(q) sm_rt[(q) * NT]
     if (SPEC) { for (int k = threadIdx.x; k < MAX_FREQ; k += NT) sm_red[k] = 0.0; }
     if (KIND == 1) { for (int k = threadIdx.x; k < P.nbins; k += NT) sm_red[k] = 0.0; }
-    if (SPEC || KIND == 1) __syncthreads();
+    if (KIND == 4) { for (int k = threadIdx.x; k < MAX_FREQ; k += NT) sm_red[k] = 0.0; }
+    if (SPEC || KIND == 1 || KIND == 4) __syncthreads();
 #define ACC(q, k) gl_acc[((q) * nf + (k)) * spec_stride]            // q: 0 tau, 1 T, 2 I, 3 a0, 4 e0
 
     const double a = P.a, a2 = P.a2;
@@ -237,7 +238,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         if (done && !fresh) {
             if (mode == M_NORMAL) {                                    // fresh accepted step: detect events
                 int m = M_NORMAL;
-                if (KIND == 1 || KIND == 3) {
+                if (KIND == 1 || KIND == 3 || KIND == 4) {
                     if (!on_eq && cos_y * cn < 0.0) m = M_EQ;          // equatorial crossing (reading P)
                     else on_eq = false;
                 }
@@ -376,6 +377,18 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                         if (b >= 0) atomicAdd(&O.hist[(size_t)k * P.nbins + b], v * P.pix_area);
                     }
                 }
+            } else if (KIND == 4) {
+                // Novikov–Thorne disk (reading NT): blackbody at T_eff(r_e), I_ν(obs) = (2hν³/c²)/expm1(hν/(g k T_eff))
+                if (O.aux0) O.aux0[pix] = g_disk;
+                if (O.aux1) O.aux1[pix] = r_e;
+                const double T = (flag == F_DISK && g_disk > 0.0) ? nt_temperature(P, r_e) : 0.0;
+                const double xk = (T > 0.0) ? P.h_over_k / (g_disk * T) : 0.0;
+                const size_t npix = (size_t)P.nx * P.ny;
+                for (int k = 0; k < P.nf; ++k) {
+                    const double v = (T > 0.0) ? P.planck2 * P.nu3[k] / expm1(P.nu[k] * xk) : 0.0;
+                    if (O.images) O.images[(size_t)k * npix + pix] = v;
+                    if (O.nuLnu && v != 0.0) atomicAdd(&sm_red[k], v);
+                }
             } else if (KIND == 1) {
                 double val = 0.0;
                 if (flag == F_DISK && g_disk > 0.0) val = pow(g_disk, P.g_power) * pow(r_e, -P.emis_index);
@@ -407,9 +420,9 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
 #undef ACC
 #undef RT1
     // ---------------------------------------------------------------------- block-level reductions
-    if (SPEC && O.nuLnu) {
+    if ((SPEC || KIND == 4) && O.nuLnu) {
         __syncthreads();
-        for (int k = threadIdx.x; k < nf; k += NT) atomicAdd(&O.nuLnu[k], P.sed_coef * P.nu[k] * sm_red[k]);
+        for (int k = threadIdx.x; k < P.nf; k += NT) atomicAdd(&O.nuLnu[k], P.sed_coef * P.nu[k] * sm_red[k]);
     }
     if (KIND == 1 && O.hist) {
         __syncthreads();

@@ -43,6 +43,12 @@ struct Params {
     // ---- hot spot (kind 3; eq. (36)); the observer times t_obs[k] travel in nu[k], nf = their number
     double spot_R, spot_Omega, spot_phi0;       // sqrt(r_s² + a²), 1/(r_s^{3/2} + a), azimuth at t = 0
     double spot_inv2s2, spot_cut2;              // 1/(2 r_spot²), (4 r_spot)²
+    // ---- Novikov–Thorne disk (kind 4; eq. (35)): Page & Thorne's f(r) in x = sqrt(r)
+    double nt_x0;                               // sqrt(r_isco)
+    double nt_x[3], nt_c[3];                    // roots of x³ - 3x + 2a and the weights 3(x_i - a)²/(x_i (x_i - x_j)(x_i - x_k))
+    double nt_T4;                               // 3 Mdot c⁶/(8π G² M² σ): T_eff⁴ = nt_T4 f / r³
+    double h_over_k;                            // h/k_B
+    double planck2;                             // 2h/c²
     double nu[MAX_FREQ];
     double ln_nu[MAX_FREQ];
     double nu12[MAX_FREQ], inu12[MAX_FREQ];     // ν^(1/12) and its reciprocal (eq. (38) in powers of x_M^(1/12))

@@ -32,7 +32,7 @@ def test_header_symbols_are_all_exported():
 def test_struct_layout_matches_header_sizes():
     # 8 doubles + 2 int32 + double + 2 int32 + 3 doubles + 2 int32 = 15*8 = 120 bytes; model: 2 int32 + 16 doubles
     assert C.sizeof(B.Scene) == 120
-    assert C.sizeof(B.Model) == 8 + 16 * 8 + 8 + 3 * 8
+    assert C.sizeof(B.Model) == 8 + 16 * 8 + 8 + 3 * 8 + 8
 
 
 @pytest.mark.parametrize("patch, msg", [
@@ -80,6 +80,12 @@ def test_invalid_model_and_frequencies_are_rejected():
     assert L.odyssey_render_hotspot(C.byref(sc), C.byref(mo), tt, 4, *([None] * 10)) == -1      # RIAF model in hot-spot mode
     bad_spot = B._struct(B.Model, W.model_hot_spot(r_spot=0.0))
     assert L.odyssey_render_hotspot(C.byref(sc), C.byref(bad_spot), tt, 4, *([None] * 10)) == -1
+    nt_bad = B._struct(B.Model, W.model_nt_disk(mbh_msun=0.0))
+    assert L.odyssey_render_spectrum(C.byref(sc), C.byref(nt_bad), nu, 4, None, None, None, None, None) == -1
+    assert "Novikov-Thorne" in ody.last_error()
+    nt = B._struct(B.Model, W.model_nt_disk())
+    assert L.odyssey_render_spectrum(C.byref(sc), C.byref(nt), nu, 33, None, None, None, None, None) == -1
+    assert L.odyssey_render_image(C.byref(sc), C.byref(nt), C.c_double(0.0), None, None, None, None, None, None, None, None) == -1
     thin = B._struct(B.Model, W.C1()["model"])
     assert L.odyssey_render_spectrum(C.byref(sc), C.byref(thin), nu, 4, None, None, None, None, None) == -1
     assert L.odyssey_render_image(None, None, C.c_double(0.0), None, None, None, None, None, None, None, None) == -1

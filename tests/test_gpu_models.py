@@ -319,3 +319,60 @@ def test_hot_spot_matches_the_oracle(ody, orc, a, incl, n, hw, kw):
     host = ody.render_hotspot_host(sc, mo, t_obs)
     assert np.array_equal(host["images"], gpu["images"]) and np.array_equal(host["t_e"], gpu["t_e"])
     assert np.allclose(host["lightcurve"], gpu["lightcurve"], rtol=1e-12)
+
+
+# ------------------------------------------------------- Novikov-Thorne disk (kind 4, eq. (35), reading NT)
+KEV_HZ = 2.417989242e17
+
+
+@pytest.mark.parametrize("a, incl, n, hw, kw", [
+    (0.999, 85.0, 128, 25.0, dict()),                                # Fig. 6's set-up: M = 10 M_sun, Mdot = 1e19 g/s, r_out = 50
+    (0.0, 45.0, 96, 60.0, dict(r_out=50.0)),
+    (0.5, 60.0, 64, 520.0, dict(r_out=500.0, mbh_msun=1.0e7, mdot_gs=1.0e24)),   # a supermassive hole: UV disk
+])
+def test_nt_disk_spectrum_matches_the_oracle(ody, orc, a, incl, n, hw, kw):
+    sc = W.scene(a, incl, n, hw)
+    mo = W.model_nt_disk(**kw)
+    t_in = orc.nt_temperature(mo, a, 1.5 * orc.kerr_constants(a)["r_isco"])
+    kt = 1.380649e-16 * t_in / 6.62607015e-27                        # k T / h of the inner disk, Hz
+    nu = list(kt * np.logspace(-3.0, 1.5, 16))
+    out = ody.render_spectrum(sc, mo, nu); _sync()
+    gpu = {k: _np(v) for k, v in out.items()}
+    ref = orc.render_spectrum(sc, mo, nu)
+    assert np.array_equal(gpu["flag"].ravel(), ref["flag"])
+    assert np.array_equal(gpu["n_attempt"].ravel(), ref["n_attempt"])
+    assert (ref["flag"] == W.FLAG_DISK).sum() > 200
+    for q in range(len(nu)):
+        _check_image(gpu["images"][q].ravel(), ref["images"][q], f"NT disk image at nu[{q}]")
+    assert np.max(np.abs(gpu["nuLnu"] - ref["nuLnu"]) / ref["nuLnu"]) <= 1e-6
+    # single-frequency image call: same pixels, plus g and r_e of the crossing
+    one = ody.render_image(sc, mo, nu[9]); _sync()
+    assert np.array_equal(_np(one["image"]), gpu["images"][9])
+    thin = orc.render_image(sc, W.model_thin_disk(r_in=mo["r_in"], r_out=mo["r_out"]))
+    hit = ref["flag"] == W.FLAG_DISK
+    g, r_e = _np(one["aux0"]).ravel(), _np(one["aux1"]).ravel()
+    assert np.max(np.abs(g[hit] - thin["aux0"][hit]) / thin["aux0"][hit]) <= 1e-8
+    assert np.max(np.abs(r_e[hit] - thin["aux1"][hit]) / thin["aux1"][hit]) <= 1e-8
+    # host entry point
+    host = ody.render_spectrum_host(sc, mo, nu)
+    assert np.array_equal(host["images"], gpu["images"])
+    assert np.allclose(host["nuLnu"], gpu["nuLnu"], rtol=1e-12)
+
+
+def test_nt_disk_degenerate_cases(ody, orc):
+    sc = W.scene(0.9, 70.0, 48, 20.0)
+    nu = [0.1 * KEV_HZ, 1.0 * KEV_HZ]
+    dark = ody.render_spectrum(sc, W.model_nt_disk(mdot_gs=0.0), nu); _sync()      # no accretion: a cold, dark disk
+    assert float(dark["images"].abs().max()) == 0.0 and float(dark["nuLnu"].abs().max()) == 0.0
+    assert int((dark["flag"] == W.FLAG_DISK).sum()) > 50
+    # a disk that reaches inside r_isco: crossings there are flagged DISK but carry no flux (f = 0)
+    mo = W.model_nt_disk(r_in=1.6, r_out=30.0)
+    out = ody.render_spectrum(sc, mo, nu); _sync()
+    ref = orc.render_spectrum(sc, mo, nu)
+    assert np.array_equal(_np(out["flag"]).ravel(), ref["flag"])
+    for q in range(2):
+        _check_image(_np(out["images"])[q].ravel(), ref["images"][q], "NT disk inside r_isco")
+    # far Wien tail: expm1 overflows to +inf and the pixel is exactly 0, on both sides
+    far = ody.render_spectrum(sc, W.model_nt_disk(), [3.0e4 * KEV_HZ]); _sync()
+    assert float(far["images"].max()) == 0.0
+    assert orc.render_spectrum(sc, W.model_nt_disk(), [3.0e4 * KEV_HZ])["images"].max() == 0.0

@@ -18,7 +18,7 @@ import math
 # Flags written per ray (same numbering on both sides; it is part of the output contract).
 FLAG_ESCAPED, FLAG_CAPTURED, FLAG_DISK, FLAG_OPAQUE, FLAG_MAXSTEP = 0, 1, 2, 3, 4
 
-KIND_NONE, KIND_THIN_DISK, KIND_RIAF, KIND_HOT_SPOT = 0, 1, 2, 3
+KIND_NONE, KIND_THIN_DISK, KIND_RIAF, KIND_HOT_SPOT, KIND_NT_DISK = 0, 1, 2, 3, 4
 # How eqs. (30), (31) are advanced (readings E, E'): one exact-attenuation update per accepted
 # step (default), or tau and I as two more Runge-Kutta components through the six stages.
 RT_PER_STEP, RT_RK_COMPONENTS = 0, 1
@@ -41,7 +41,7 @@ def model_none():
                 mbh_msun=0.0, n0=0.0, n_index=0.0, T0=0.0, T_index=0.0, h_over_r=1.0, beta=1.0,
                 r_rt_out=0.0, tau_max=0.0, j_scale=1.0,
                 nbins=0, g_lo=0.0, g_hi=1.0, g_power=0.0, rt_scheme=RT_PER_STEP,
-                spot_r_orbit=0.0, spot_size=0.0, spot_phi0=0.0)
+                spot_r_orbit=0.0, spot_size=0.0, spot_phi0=0.0, mdot_gs=0.0)
 
 
 def model_thin_disk(r_in=0.0, r_out=50.0, emis_index=3.0, nbins=200, g_lo=0.0, g_hi=2.0, g_power=3.0):
@@ -59,6 +59,14 @@ def model_hot_spot(r_orbit=0.0, r_spot=0.5, phi0=0.0, r_in=0.0, r_out=50.0, g_po
     m = model_none()
     m.update(kind=KIND_HOT_SPOT, r_in=float(r_in), r_out=float(r_out), g_power=float(g_power), nbins=int(nbins),
              g_lo=float(g_lo), g_hi=float(g_hi), spot_r_orbit=float(r_orbit), spot_size=float(r_spot), spot_phi0=float(phi0))
+    return m
+
+
+def model_nt_disk(mbh_msun=10.0, mdot_gs=1.0e19, r_in=0.0, r_out=50.0):
+    """Novikov-Thorne multi-temperature disk, eq. (35) (Fig. 6 uses M = 10 M_sun,
+    Mdot = 1e19 g/s, r_out = 50 or 500 r_g)."""
+    m = model_none()
+    m.update(kind=KIND_NT_DISK, mbh_msun=float(mbh_msun), mdot_gs=float(mdot_gs), r_in=float(r_in), r_out=float(r_out))
     return m
 
 
