@@ -63,6 +63,12 @@ def main():
     # the set-up of the paper's own timing table (Table 1: geodesics only, a = 0.95, i = 60 deg,
     # 1024^2; the image-plane extent is not stated there: +/-10 M is used)
     cases.append(("paper Table 1 set-up: geodesics only a=0.95 i=60 1024^2", dict(scene=W.scene(0.95, 60.0, 1024, 10.0), model=W.model_none(), nu=[])))
+    # Fig. 6's set-up: Novikov-Thorne disk, a = 0.999, i = 85 deg, M = 10 M_sun, Mdot = 1e19 g/s,
+    # r_out = 500 r_g; 32 photon energies 0.01-30 keV
+    kev = 2.417989242e17
+    cases.append(("Fig. 6 set-up: Novikov-Thorne disk a=0.999 i=85 r_out=500, 1024^2 x 32 energies",
+                  dict(scene=W.scene(0.999, 85.0, 1024, 520.0), model=W.model_nt_disk(r_out=500.0),
+                       nu=W.log_spaced_frequencies(0.01 * kev, 30.0 * kev, 32))))
     if args.sweep:
         for a in (0.0, 0.5, 0.9, 0.998):
             for n in (1024, 2048, 4096):
