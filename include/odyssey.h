@@ -83,7 +83,7 @@ typedef struct odyssey_scene {
     int32_t tableau, pad0;     /* ODYSSEY_TABLEAU_*                                              */
     double h0;                 /* first trial step in affine parameter                           */
     double horizon_eps;        /* capture radius = r_h + horizon_eps                             */
-    double r_esc;              /* escape radius                                                  */
+    double r_esc;              /* escape radius; the image-plane corners must satisfy sqrt(x^2 + y^2) <= 0.9 r_esc */
     int32_t max_attempts, pad1;
 } odyssey_scene;
 

@@ -93,6 +93,13 @@ int check_scene(const odyssey_scene* S) {
         return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "r_obs, h0, r_esc, max_attempts must be positive and horizon_eps >= 0");
     if (!(S->x_max > S->x_min) || !(S->y_max > S->y_min))
         return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "image-plane extent is empty");
+    {   // every ray must come back out through r = r_esc: a ray whose impact parameter exceeds r_esc turns around
+        // outside the escape sphere and its "escape point" (located by Newton iteration on r = r_esc) does not exist
+        const double xm = std::fmax(std::fabs(S->x_min), std::fabs(S->x_max)), ym = std::fmax(std::fabs(S->y_min), std::fabs(S->y_max));
+        const double b_corner = std::sqrt(xm * xm + ym * ym);
+        if (!(b_corner <= 0.9 * S->r_esc))
+            return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "image-plane extent: corner impact parameter %g exceeds 0.9 r_esc = %g", b_corner, 0.9 * S->r_esc);
+    }
     return ODYSSEY_OK;
 }
 
