@@ -36,7 +36,7 @@ def test_struct_layout_matches_header_sizes():
 
 
 @pytest.mark.parametrize("patch, msg", [
-    (dict(a=1.0), "spin"), (dict(nx=0), "nx"), (dict(rtol=0.0), "rtol"), (dict(tableau=7), "tableau"),
+    (dict(a=1.0), "spin"), (dict(nx=0), "nx"), (dict(nx=32769, ny=32768), "2^30"), (dict(rtol=0.0), "rtol"), (dict(tableau=7), "tableau"),
     (dict(x_max=-10.0), "extent"), (dict(max_attempts=0), "max_attempts"),
     (dict(x_min=-2000.0, x_max=2000.0), "r_esc"), (dict(r_obs=50.0, r_esc=55.0, y_min=-300.0, y_max=300.0), "r_esc"),
 ])

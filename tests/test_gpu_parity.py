@@ -231,3 +231,29 @@ def test_near_polar_observers_within_the_conditioning_limit(ody, orc, a, incl):
         assert e.max() <= 1e-6, (k, e.max())
         errs.append(e)
     assert np.median(np.maximum.reduce(errs)) <= 1e-10
+
+
+def test_maximum_image_size_two_to_the_thirty_pixels(ody, orc):
+    # the largest image the ABI accepts (include/odyssey.h: nx * ny <= 2^30): every pixel written, and pixels at the
+    # corners, edges and middle equal to the oracle's (64-bit indexing of the queue, the camera scratch, the outputs)
+    import ctypes as C
+    import torch
+    from paper_1601_02063_b200 import binding as B
+    n = 32768
+    sc = W.scene(0.9, 60.0, n, 12.0)
+    flag = torch.full((n, n), -7, dtype=torch.int32, device="cuda")
+    natt = torch.empty((n, n), dtype=torch.int32, device="cuda")
+    r = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    rc = ody.load_library().odyssey_trace_geodesics(C.byref(B._struct(B.Scene, sc)), B._ptr(flag), B._ptr(r), None, None, None,
+                                                    B._ptr(natt), None, None)
+    _sync()
+    assert rc == 0, ody.last_error()
+    assert int((flag == -7).sum()) == 0
+    ii = np.array([0, 1, n // 2 - 1, n // 2, n - 1, 12345, n - 7] * 3)
+    jj = np.array([0] * 7 + [n - 1] * 7 + [n // 2 + 3] * 7)
+    ref = orc.trace_geodesics(sc, idx=(list(ii), list(jj)))
+    assert np.array_equal(flag[jj, ii].cpu().numpy(), ref["flag"])
+    assert np.array_equal(natt[jj, ii].cpu().numpy(), ref["n_attempt"])
+    assert np.max(np.abs(r[jj, ii].cpu().numpy() - ref["r"]) / ref["r"]) <= 1e-8
+    del flag, natt, r
+    torch.cuda.empty_cache()
