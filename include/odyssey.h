@@ -108,6 +108,9 @@ typedef struct odyssey_model {
     double spot_size;          /* kind 3: r_spot of eq. (36) (the paper uses 0.5 r_g); emission is cut at 4 r_spot */
     double spot_phi0;          /* kind 3: azimuth of the spot centre at coordinate time t = 0                    */
     double mdot_gs;            /* kind 4: accretion rate in g/s (eq. (35)); uses mbh_msun, r_in (<= 0: r_isco), r_out */
+    double dtau_max;           /* kind 2, ODYSSEY_RT_PER_STEP, FP64, odyssey_render_image only: > 0 caps the step that follows an
+                                  accepted step at dtau_max optical depths, h <= dtau_max / (absorption coefficient at the point
+                                  just reached); <= 0: no cap (the default; the step is controlled by the geodesic alone)   */
 } odyssey_model;
 
 /* Geodesics only (BASELINE.json:configs[0]; §2.1-2.2).  Per pixel: outcome flag, the

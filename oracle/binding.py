@@ -33,7 +33,7 @@ class Model(C.Structure):
                 ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double),
                 ("rt_scheme", C.c_int32), ("pad", C.c_int32),
                 ("spot_r_orbit", C.c_double), ("spot_size", C.c_double), ("spot_phi0", C.c_double),
-                ("mdot_gs", C.c_double)]
+                ("mdot_gs", C.c_double), ("dtau_max", C.c_double)]
 
 
 def _fill(struct, d):
@@ -219,6 +219,15 @@ def trace_path(scene, model, x, y, max_nodes=20000):
                                 C.c_int(max_nodes), _dp(nodes), _dp(cons), _ip(res))
     return nodes[:min(n, max_nodes)], dict(E=cons[0], L=cons[1], Q=cons[2]), dict(flag=int(res[0]), n_attempt=int(res[1]),
                                                                                    n_accept=int(res[2]))
+
+
+def trace_path_rt(scene, model, nu_hz, x, y, max_nodes=20000):
+    """trace_path with the transfer at one frequency: also the absorption coefficient at each node."""
+    nodes = np.zeros((max_nodes, 7)); absorb = np.zeros(max_nodes); res = np.zeros(3, np.int32)
+    n = lib().oracle_trace_path_rt(C.byref(make_scene(scene)), C.byref(make_model(model)), C.c_double(nu_hz),
+                                   C.c_double(x), C.c_double(y), C.c_int(max_nodes), _dp(nodes), _dp(absorb), _ip(res))
+    n = min(n, max_nodes)
+    return nodes[:n], absorb[:n], dict(flag=int(res[0]), n_attempt=int(res[1]), n_accept=int(res[2]))
 
 
 def _pixels(scene, idx):

@@ -79,6 +79,7 @@ struct Model {           // mirrors workloads.model_*()
     int32_t rt_scheme, pad;  // 0: one update per accepted step [reading E]; 1: tau, I as Runge-Kutta components [E']
     double spot_r_orbit, spot_size, spot_phi0;   // kind 3 [reading HS]: orbit radius (<= 0: r_isco), r_spot, azimuth at t = 0
     double mdot_gs;                              // kind 4 [reading NT]: accretion rate, g/s
+    double dtau_max;                             // kind 2, rt_scheme 0 [reading DT]: cap of the next step's optical depth (<= 0: off)
 };
 
 // ----------------------------------------------------------------------------------------------
@@ -425,7 +426,10 @@ struct RayOut {
     std::vector<double> I, tau;          // invariant intensity I_nu/nu^3 and optical depth per frequency
 };
 
-struct Path { std::vector<double> nodes; };   // per accepted node: (r, theta, phi, p_r, p_theta), the affine parameter, t
+struct Path {
+    std::vector<double> nodes;   // per accepted node: (r, theta, phi, p_r, p_theta), the affine parameter, t
+    std::vector<double> absorb;  // per accepted node: invariant absorption coefficient of frequency 0 there (kind 2, nf >= 1)
+};
 
 constexpr int LOCATE_MAX = 8;
 
@@ -444,7 +448,7 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
     double g = 0.0, r_e = 0.0;
     if (M.kind == 2) rt_coefficients(S, M, F, ray, y, nf, nu, a0.data(), e0.data());
     double lambda = 0.0;
-    if (path) { path->nodes.insert(path->nodes.end(), y, y + 5); path->nodes.push_back(lambda); path->nodes.push_back(y[5]); }
+    if (path) { path->nodes.insert(path->nodes.end(), y, y + 5); path->nodes.push_back(lambda); path->nodes.push_back(y[5]); if (nf > 0) path->absorb.push_back(a0[0]); }
 
     while (flag < 0) {
         if (n_attempt >= S.max_attempts) { flag = MAXSTEP; break; }
@@ -505,6 +509,14 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
             }
             a0.swap(a1); e0.swap(e1);
             if (flag < 0 && all_opaque) flag = OPAQUE;
+            // [reading DT, SURVEY §8(f)-2 "a Δτ-limited step cap"]: the next step may not be longer than dtau_max
+            // optical depths at the absorption coefficient of the point just reached (largest over the frequencies
+            // still being integrated)
+            if (M.dtau_max > 0.0) {
+                double amax = 0.0;
+                for (int k = 0; k < nf; ++k) if (!(tau[k] > M.tau_max)) amax = std::max(amax, a0[k]);
+                if (amax > 0.0) h_next = std::min(h_next, M.dtau_max / amax);
+            }
         } else if (M.kind == 2) {                       // [E']: coefficients at the six stage states of the step taken
             std::vector<double> as(6 * (size_t)nf), es(6 * (size_t)nf);
             for (int i = 0; i < 6; ++i)
@@ -521,7 +533,7 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
         for (int v = 0; v < NV; ++v) y[v] = ynew[v];
         h = h_next;
         lambda += h_used;
-        if (path) { path->nodes.insert(path->nodes.end(), y, y + 5); path->nodes.push_back(lambda); path->nodes.push_back(y[5]); }
+        if (path) { path->nodes.insert(path->nodes.end(), y, y + 5); path->nodes.push_back(lambda); path->nodes.push_back(y[5]); if (nf > 0) path->absorb.push_back(a0[0]); }
     }
     out->flag = flag; out->r = y[0]; out->th = y[1]; out->ph = y[2]; out->t = y[5];
     out->n_attempt = n_attempt; out->n_accept = n_accept;
@@ -746,6 +758,20 @@ int oracle_trace_path(const Scene* S, const Model* M, double x, double y, int ma
     int n = (int)(P.nodes.size() / 7);
     int m = std::min(n, max_nodes);
     std::memcpy(nodes, P.nodes.data(), sizeof(double) * 7 * (size_t)m);
+    res[0] = R.flag; res[1] = R.n_attempt; res[2] = R.n_accept;
+    return n;
+}
+
+// The same with the transfer at one frequency along the ray (kind 2): absorb[n] = the invariant absorption
+// coefficient at each node (what the Δτ cap of reading DT looks at); res = {flag, n_attempt, n_accept}.
+int oracle_trace_path_rt(const Scene* S, const Model* M, double nu_hz, double x, double y, int max_nodes,
+                         double* nodes, double* absorb, int32_t* res) {
+    RayOut R; Path P;
+    trace_ray(*S, *M, 1, &nu_hz, x, y, &R, &P);
+    int n = (int)(P.nodes.size() / 7);
+    int m = std::min(n, max_nodes);
+    std::memcpy(nodes, P.nodes.data(), sizeof(double) * 7 * (size_t)m);
+    for (int k = 0; k < m && k < (int)P.absorb.size(); ++k) absorb[k] = P.absorb[k];
     res[0] = R.flag; res[1] = R.n_attempt; res[2] = R.n_accept;
     return n;
 }

@@ -46,7 +46,7 @@ class Model(C.Structure):
                 ("g_lo", C.c_double), ("g_hi", C.c_double), ("g_power", C.c_double),
                 ("rt_scheme", C.c_int32), ("precision", C.c_int32),
                 ("spot_r_orbit", C.c_double), ("spot_size", C.c_double), ("spot_phi0", C.c_double),
-                ("mdot_gs", C.c_double)]
+                ("mdot_gs", C.c_double), ("dtau_max", C.c_double)]
 
 
 def _struct(cls, d):

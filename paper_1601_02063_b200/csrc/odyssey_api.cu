@@ -126,6 +126,8 @@ int check_model(const odyssey_model* M) {
             return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown precision %d", M->precision);
         if (M->precision == ODYSSEY_PREC_MIXED_FP32 && M->rt_scheme != ODYSSEY_RT_PER_STEP)
             return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "precision MIXED_FP32 needs rt_scheme PER_STEP");
+        if (M->dtau_max > 0.0 && (M->rt_scheme != ODYSSEY_RT_PER_STEP || M->precision != ODYSSEY_PREC_FP64))
+            return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "dtau_max > 0 needs rt_scheme PER_STEP and precision FP64");
         if (!(M->mbh_msun > 0.0) || !(M->h_over_r > 0.0) || !(M->beta > 0.0) || !(M->T0 > 0.0) || !(M->n0 >= 0.0) ||
             !(M->j_scale >= 0.0))
             return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "RIAF parameters mbh_msun, h_over_r, beta, T0 must be positive, n0 and j_scale non-negative");
@@ -204,6 +206,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
         P->h_over_mc2 = kH / (kMe * kC * kC);
         P->inv_planck = kC * kC / (2.0 * kH);
         P->r_rt_out = M->r_rt_out; P->tau_max = M->tau_max; P->rt_scheme = M->rt_scheme; P->precision = M->precision;
+        if (M->dtau_max > 0.0) { P->rt_scheme = 3; P->dtau_max = M->dtau_max; }
         P->rg_cm = kGMsun * M->mbh_msun / (kC * kC);
         P->sed_coef = 4.0 * kPi * P->rg_cm * P->rg_cm * P->pix_area;
         for (int k = 0; k < nf && k < MAX_FREQ; ++k) { P->nu[k] = nu[k]; P->ln_nu[k] = std::log(nu[k]); P->nu12[k] = std::exp(P->ln_nu[k] / 12.0); P->inu12[k] = 1.0 / P->nu12[k]; P->nu3[k] = nu[k] * nu[k] * nu[k]; }
@@ -229,6 +232,8 @@ KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0, int prec = 0, bo
         return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_MAIN, 0, 1> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_MAIN, 0, 1>;
     if (kind == 2 && !spec && rts == 1)
         return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_RK, 1> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_RK, 1>;
+    if (kind == 2 && !spec && rts == 3)
+        return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_MAIN, 3> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_MAIN, 3>;
     if (kind == 2 && !spec && rts == 2)
         return tab ? odyssey_kernel<2, 1, false, NT_MAIN, 4, 2> : odyssey_kernel<2, 0, false, NT_MAIN, 4, 2>;
     if (spec) return tab ? odyssey_kernel<2, 1, true, NT_SPEC, MINB_SPEC> : odyssey_kernel<2, 0, true, NT_SPEC, MINB_SPEC>;
@@ -477,6 +482,7 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
         return launch(P, O, false, scene->tableau, (cudaStream_t)cuda_stream);      // one geodesic pass, all frequencies at the crossing
     }
     if (model->rt_scheme != ODYSSEY_RT_PER_STEP) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode supports rt_scheme 0 (per-step update) only");
+    if (model->dtau_max > 0.0) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode does not support dtau_max (single-frequency image calls only)");
     if (model->precision != ODYSSEY_PREC_FP64) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spectrum mode supports precision FP64 only");
     if (nf < 1 || nf > ODYSSEY_MAX_FREQ) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nf = %d outside [1, %d]", nf, ODYSSEY_MAX_FREQ);
     if (!nu_hz_host) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nu_hz_host is NULL");

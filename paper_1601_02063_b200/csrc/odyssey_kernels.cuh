@@ -60,6 +60,7 @@ __host__ __device__ constexpr int smem_per_thread(int rts) { return (rts == 1 ? 
 
 // RTS = 1: transfer scheme E' (tau, I as Runge–Kutta components; single frequency only).
 // RTS = 2: record mode, the first phase of the two-phase spectrum path (see spectrum_rt_kernel below).
+// RTS = 3: the per-step scheme with the optical-depth cap on the next step (reading DT; single frequency only).
 // PREC = 1: mixed-precision transfer (FP32 polynomial cores; single frequency, per-step scheme only).
 // TIME = 1: also integrate the coordinate time t of eq. (9) (it is not in the error norm) and write it to O.t.
 template <int KIND, int TAB, bool SPEC, int NT, int MINB, int RTS = 0, int PREC = 0, int TIME = 0>
@@ -321,6 +322,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     rt_update<PREC>(RT1(3), a1, RT1(4), e1, h_try, P.tau_max, tau, Tr, Inu);
                     RT1(0) = tau; RT1(1) = Tr; RT1(2) = Inu;
                     all_opaque = (tau > P.tau_max);
+                    // reading DT: the next step is at most dtau_max optical depths long at the coefficient just reached
+                    if (RTS == 3 && !all_opaque && a1 > 0.0) h_next = fmin(h_next, P.dtau_max / a1);
                 }
                 RT1(3) = a1; RT1(4) = e1;
             }

@@ -38,7 +38,8 @@ struct Params {
     double inv_planck;                          // c²/(2h)
     double r_rt_out, tau_max, rg_cm;
     double sed_coef;                            // 4π r_g^2 Δx Δy
-    int32_t nf, rt_scheme;                      // rt_scheme: ODYSSEY_RT_* (kind 2)
+    int32_t nf, rt_scheme;                      // rt_scheme: ODYSSEY_RT_* (kind 2); internally 2 = record pass, 3 = per-step with the Δτ cap
+    double dtau_max;                            // (rt_scheme 3) cap of the next step's optical depth
     int32_t precision, pad3;                    // ODYSSEY_PREC_* (kind 2)
     // ---- hot spot (kind 3; eq. (36)); the observer times t_obs[k] travel in nu[k], nf = their number
     double spot_R, spot_Omega, spot_phi0;       // sqrt(r_s² + a²), 1/(r_s^{3/2} + a), azimuth at t = 0

@@ -32,7 +32,7 @@ def test_header_symbols_are_all_exported():
 def test_struct_layout_matches_header_sizes():
     # 8 doubles + 2 int32 + double + 2 int32 + 3 doubles + 2 int32 = 15*8 = 120 bytes; model: 2 int32 + 16 doubles
     assert C.sizeof(B.Scene) == 120
-    assert C.sizeof(B.Model) == 8 + 16 * 8 + 8 + 3 * 8 + 8
+    assert C.sizeof(B.Model) == 8 + 16 * 8 + 8 + 3 * 8 + 8 + 8
 
 
 @pytest.mark.parametrize("patch, msg", [
@@ -72,6 +72,13 @@ def test_invalid_model_and_frequencies_are_rejected():
     mixed = B._struct(B.Model, w["model"]); mixed.precision = 1
     assert L.odyssey_render_spectrum(C.byref(sc), C.byref(mixed), nu, 4, None, None, None, None, None) == -1
     assert "precision" in ody.last_error()
+    capped = B._struct(B.Model, W.model_riaf(dtau_max=0.1))
+    assert L.odyssey_render_spectrum(C.byref(sc), C.byref(capped), nu, 4, None, None, None, None, None) == -1
+    assert "dtau_max" in ody.last_error()
+    capped_rk = B._struct(B.Model, W.model_riaf(dtau_max=0.1, rt_scheme=W.RT_RK_COMPONENTS))
+    assert L.odyssey_render_image(C.byref(sc), C.byref(capped_rk), C.c_double(1e9),
+                                  None, None, None, None, None, None, None, None) == -1
+    assert "dtau_max" in ody.last_error()
     spot = B._struct(B.Model, W.model_hot_spot())
     assert L.odyssey_render_image(C.byref(sc), C.byref(spot), C.c_double(1e9),
                                   None, None, None, None, None, None, None, None) == -1

@@ -376,3 +376,26 @@ def test_nt_disk_degenerate_cases(ody, orc):
     far = ody.render_spectrum(sc, W.model_nt_disk(), [3.0e4 * KEV_HZ]); _sync()
     assert float(far["images"].max()) == 0.0
     assert orc.render_spectrum(sc, W.model_nt_disk(), [3.0e4 * KEV_HZ])["images"].max() == 0.0
+
+
+# ------------------------------------------------- optical-depth step cap (reading DT)
+@pytest.mark.parametrize("nu, cap, tableau", [(1.0e10, 0.1, W.TABLEAU_RKF45), (1.0e10, 0.5, W.TABLEAU_CASH_KARP),
+                                             (5.0e10, 0.02, W.TABLEAU_RKF45), (2.3e11, 0.05, W.TABLEAU_RKF45)])
+def test_dtau_step_cap_matches_the_oracle(ody, orc, nu, cap, tableau):
+    w = W.C2(n=96)
+    sc = dict(w["scene"]); sc["tableau"] = tableau
+    mo = W.model_riaf(dtau_max=cap)
+    out = ody.render_image(sc, mo, nu); _sync()
+    ref = orc.render_image(sc, mo, nu)
+    assert np.array_equal(_np(out["flag"]).ravel(), ref["flag"])
+    assert np.mean(_np(out["n_attempt"]).ravel() == ref["n_attempt"]) >= 0.995
+    _check_image(_np(out["image"]).ravel(), ref["image"], "image with the optical-depth cap")
+    tau, tau_ref = _np(out["aux0"]).ravel(), ref["aux0"]
+    assert np.max(np.abs(tau - tau_ref) / np.maximum(tau_ref, 1e-30)) <= 1e-6
+    # the cap binds in the thick cases: more steps than without it; it is inert where tau stays below it
+    free = ody.render_image(sc, W.model_riaf(), nu); _sync()
+    n_cap, n_free = int(out["n_attempt"].sum()), int(free["n_attempt"].sum())
+    if float(free["aux0"].max()) < cap:
+        assert n_cap == n_free and bool((out["image"] == free["image"]).all())
+    else:
+        assert n_cap > n_free

@@ -41,7 +41,7 @@ def model_none():
                 mbh_msun=0.0, n0=0.0, n_index=0.0, T0=0.0, T_index=0.0, h_over_r=1.0, beta=1.0,
                 r_rt_out=0.0, tau_max=0.0, j_scale=1.0,
                 nbins=0, g_lo=0.0, g_hi=1.0, g_power=0.0, rt_scheme=RT_PER_STEP,
-                spot_r_orbit=0.0, spot_size=0.0, spot_phi0=0.0, mdot_gs=0.0)
+                spot_r_orbit=0.0, spot_size=0.0, spot_phi0=0.0, mdot_gs=0.0, dtau_max=0.0)
 
 
 def model_thin_disk(r_in=0.0, r_out=50.0, emis_index=3.0, nbins=200, g_lo=0.0, g_hi=2.0, g_power=3.0):
@@ -71,12 +71,13 @@ def model_nt_disk(mbh_msun=10.0, mdot_gs=1.0e19, r_in=0.0, r_out=50.0):
 
 
 def model_riaf(mbh_msun=4.0e6, n0=1.0e7, n_index=-1.1, T0=1.0e11, T_index=-0.84, h_over_r=0.3,
-               beta=10.0, r_rt_out=500.0, tau_max=30.0, j_scale=1.0, rt_scheme=RT_PER_STEP):
+               beta=10.0, r_rt_out=500.0, tau_max=30.0, j_scale=1.0, rt_scheme=RT_PER_STEP, dtau_max=0.0):
     """Analytic RIAF-like flow of BASELINE.json:configs[2]; mass and outer radius from PAPER.md:L292."""
     m = model_none()
     m.update(kind=KIND_RIAF, mbh_msun=float(mbh_msun), n0=float(n0), n_index=float(n_index),
              T0=float(T0), T_index=float(T_index), h_over_r=float(h_over_r), beta=float(beta),
-             r_rt_out=float(r_rt_out), tau_max=float(tau_max), j_scale=float(j_scale), rt_scheme=int(rt_scheme))
+             r_rt_out=float(r_rt_out), tau_max=float(tau_max), j_scale=float(j_scale), rt_scheme=int(rt_scheme),
+             dtau_max=float(dtau_max))
     return m
 
 
