@@ -392,10 +392,11 @@ def test_dtau_step_cap_matches_the_oracle(ody, orc, nu, cap, tableau):
     _check_image(_np(out["image"]).ravel(), ref["image"], "image with the optical-depth cap")
     tau, tau_ref = _np(out["aux0"]).ravel(), ref["aux0"]
     assert np.max(np.abs(tau - tau_ref) / np.maximum(tau_ref, 1e-30)) <= 1e-6
-    # the cap binds in the thick cases: more steps than without it; it is inert where tau stays below it
+    # the cap binds in the optically thick cases (many more steps); at 230 GHz (tau <= 0.3 in total) hardly any step
+    # is longer than 0.05 optical depths and the step count barely moves
     free = ody.render_image(sc, W.model_riaf(), nu); _sync()
     n_cap, n_free = int(out["n_attempt"].sum()), int(free["n_attempt"].sum())
-    if float(free["aux0"].max()) < cap:
-        assert n_cap == n_free and bool((out["image"] == free["image"]).all())
+    if nu <= 5.0e10:
+        assert n_cap > 1.05 * n_free
     else:
-        assert n_cap > n_free
+        assert abs(n_cap - n_free) <= 1e-3 * n_free
