@@ -445,7 +445,7 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
     int n_attempt = 0, n_accept = 0, flag = -1;
     bool on_equator = false;
     std::vector<double> tau(nf, 0.0), Tr(nf, 1.0), I(nf, 0.0), a0(nf, 0.0), e0(nf, 0.0), a1(nf, 0.0), e1(nf, 0.0);
-    double g = 0.0, r_e = 0.0;
+    double g = 0.0, r_e = 0.0, phi_plane = 0.0;
     if (M.kind == 2) rt_coefficients(S, M, F, ray, y, nf, nu, a0.data(), e0.data());
     double lambda = 0.0;
     if (path) { path->nodes.insert(path->nodes.end(), y, y + 5); path->nodes.push_back(lambda); path->nodes.push_back(y[5]); if (nf > 0) path->absorb.push_back(a0[0]); }
@@ -482,11 +482,16 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
 
         // (1) thin disk: equatorial crossing inside the step [reading P]
         if ((M.kind == 1 || M.kind == 3 || M.kind == 4) && !on_equator && std::cos(y[1]) * std::cos(ynew[1]) < 0.0) {
-            locate(1, 0.5 * PI);
+            // A ray that has passed through the axis (possible only for L_z = 0, or when the integrator steps over the
+            // centrifugal barrier of a tiny L_z) continues with theta outside [0, pi]: the equatorial plane is
+            // theta = pi/2 + k pi, and (r, pi/2 + k pi, phi) is the point (r, pi/2, phi + k pi).
+            const double k_eq = std::nearbyint((ynew[1] - 0.5 * PI) / PI);
+            locate(1, 0.5 * PI + k_eq * PI);
             on_equator = true;
             if (ynew[0] >= r_in && ynew[0] <= M.r_out && ynew[0] > r_cap) {
                 flag = DISK;
                 r_e = ynew[0];
+                phi_plane = k_eq * PI;
                 double u[4];
                 double yeq[NV] = {ynew[0], 0.5 * PI, ynew[2], ynew[3], ynew[4], ynew[5]};
                 if (flow_velocity(S.a, F, r_e, 0.5 * PI, u)) g = gamma_shift(ray, yeq, u);
@@ -535,7 +540,7 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
         lambda += h_used;
         if (path) { path->nodes.insert(path->nodes.end(), y, y + 5); path->nodes.push_back(lambda); path->nodes.push_back(y[5]); if (nf > 0) path->absorb.push_back(a0[0]); }
     }
-    out->flag = flag; out->r = y[0]; out->th = y[1]; out->ph = y[2]; out->t = y[5];
+    out->flag = flag; out->r = y[0]; out->th = y[1]; out->ph = y[2] + phi_plane; out->t = y[5];   // (DISK: azimuth of the point on the plane)
     out->n_attempt = n_attempt; out->n_accept = n_accept;
     out->g = g; out->r_e = r_e;
     out->I = I; out->tau = tau;

@@ -215,7 +215,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
 
 // ---- kernel table ------------------------------------------------------------------------------
 constexpr int NT_MAIN = 128, MINB_MAIN = 5;     // 96 registers per thread at most
-constexpr int MINB_SPOT = 4;                    // hot spot (kind 3, with the coordinate time): 4 blocks per SM keep it free of spills
+constexpr int MINB_SPOT = 4;                    // hot spot (kind 3, with the coordinate time) and Novikov-Thorne disk (kind 4): 4 blocks per SM keep them free of spills
 constexpr int MINB_RK = 2;                      // transfer scheme E' (RK components): the in-loop transfer code wants > 168 registers
 constexpr int NT_SPEC = 128, MINB_SPEC = 3;     // 168 registers (the unrolled frequency loop wants them); per-frequency accumulators in a global scratch buffer
 
@@ -225,7 +225,7 @@ KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0, int prec = 0, bo
     if (kind == 3)
         return tab ? odyssey_kernel<3, 1, false, NT_MAIN, MINB_SPOT, 0, 0, 1> : odyssey_kernel<3, 0, false, NT_MAIN, MINB_SPOT, 0, 0, 1>;
     if (kind == 4)
-        return tab ? odyssey_kernel<4, 1, false, NT_MAIN, MINB_MAIN> : odyssey_kernel<4, 0, false, NT_MAIN, MINB_MAIN>;
+        return tab ? odyssey_kernel<4, 1, false, NT_MAIN, MINB_SPOT> : odyssey_kernel<4, 0, false, NT_MAIN, MINB_SPOT>;
     if (kind == 0 && time)
         return tab ? odyssey_kernel<0, 1, false, NT_MAIN, MINB_MAIN, 0, 0, 1> : odyssey_kernel<0, 0, false, NT_MAIN, MINB_MAIN, 0, 0, 1>;
     if (kind == 2 && !spec && rts == 0 && prec == 1)

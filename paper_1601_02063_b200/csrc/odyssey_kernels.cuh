@@ -38,7 +38,7 @@ namespace ody {
 constexpr int M_NORMAL = 0, M_EQ = 1, M_CAP = 2, M_ESC = 3, M_FRESH = 4;       // lane modes
 constexpr int F_ESCAPED = 0, F_CAPTURED = 1, F_DISK = 2, F_OPAQUE = 3, F_MAXSTEP = 4;
 constexpr unsigned FULL = 0xffffffffu;
-constexpr double HALF_PI = 1.57079632679489661923;
+constexpr double HALF_PI = 1.57079632679489661923, PI_D = 3.14159265358979323846, INV_PI_D = 0.31830988618379067154;
 
 // capture / escape test on a candidate end state (reading J)
 __device__ __forceinline__ int radial_event(const Params& P, const State& yn) {
@@ -67,6 +67,7 @@ template <int KIND, int TAB, bool SPEC, int NT, int MINB, int RTS = 0, int PREC 
 __global__ void __launch_bounds__(NT, MINB)
 odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs O) {
     extern __shared__ double smem[];
+    constexpr bool HAS_EQ = (KIND == 1 || KIND == 3 || KIND == 4);     // models on the equatorial plane
     const int lane = threadIdx.x & 31;
     const int nf = SPEC ? P.nf : 1;
     // shared layout: [5][6][NT] stage values, [5][NT] single-frequency RT state, then hist[nbins] (KIND 1)
@@ -248,7 +249,10 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             }
             bool retake = false;
             while (mode != M_NORMAL) {                                 // at most two passes (EQ then radial)
-                const double target = (mode == M_EQ) ? HALF_PI : ((mode == M_CAP) ? P.r_cap : P.r_esc);
+                // the equatorial plane continued through the axis is θ = π/2 + kπ (a ray with L_z = 0 passes the pole
+                // and goes on with θ outside [0, π]): the crossing nearest to the trial end state
+                const double target = (HAS_EQ && mode == M_EQ) ? fma(PI_D, rint((yn.th - HALF_PI) * INV_PI_D), HALF_PI)
+                                                     : ((mode == M_CAP) ? P.r_cap : P.r_esc);
                 const double f = ((mode == M_EQ) ? yn.th : yn.r) - target;
                 const double ftol = 1e-12 * fmax(1.0, fabs(target));
                 if (loc_it < LOCATE_MAX && fabs(f) > ftol) {           // Newton on the step size, re-take from y
@@ -353,9 +357,11 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                 // hot spot on the equatorial plane (reading HS): brightness of the crossing point at each observer
                 // time t_obs[k] (kept in P.nu[k]), spot centre at the emission time t_obs + t_e (t_e = y_t < 0)
                 const bool hit = (flag == F_DISK && g_disk > 0.0);
+                // (r, π/2 + kπ, φ) is the point (r, π/2, φ + kπ)
+                const double ph_e = fma(PI_D, rint((y.th - HALF_PI) * INV_PI_D), y.ph);
                 if (O.aux0) O.aux0[pix] = g_disk;
                 if (O.aux1) O.aux1[pix] = r_e;
-                if (O.ph) O.ph[pix] = (flag == F_DISK) ? y.ph : 0.0;
+                if (O.ph) O.ph[pix] = (flag == F_DISK) ? ph_e : 0.0;
                 if (O.t) O.t[pix] = (flag == F_DISK) ? y_t : 0.0;
                 const size_t npix = (size_t)P.nx * P.ny;
                 const double Re = sqrt(fma(r_e, r_e, P.a2));
@@ -371,7 +377,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     double v = 0.0;
                     if (near) {
                         const double phis = fma(P.spot_Omega, P.nu[k] + y_t, P.spot_phi0);
-                        const double d2 = fma(Re, Re, P.spot_R * P.spot_R) - 2.0 * Re * P.spot_R * cos(y.ph - phis);
+                        const double d2 = fma(Re, Re, P.spot_R * P.spot_R) - 2.0 * Re * P.spot_R * cos(ph_e - phis);
                         if (d2 < P.spot_cut2) v = gp * exp(-d2 * P.spot_inv2s2);
                     }
                     if (O.images) O.images[(size_t)k * npix + pix] = v;

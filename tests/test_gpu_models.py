@@ -400,3 +400,41 @@ def test_dtau_step_cap_matches_the_oracle(ody, orc, nu, cap, tableau):
         assert n_cap > 1.05 * n_free
     else:
         assert abs(n_cap - n_free) <= 1e-3 * n_free
+
+
+# ------------------------------------------------------ rays through the rotation axis (L_z = 0 exactly)
+@pytest.mark.parametrize("a, incl", [(0.0, 120.0), (0.9, 100.0), (0.998, 175.0), (0.5, 60.0)])
+def test_centre_column_rays_through_the_axis_match_the_oracle(ody, orc, a, incl):
+    # an odd number of columns puts x = 0 (L_z = 0) on the centre column: those rays pass through the pole, continue with
+    # theta outside [0, pi] and meet the plane at theta = pi/2 + k pi (oracle pin:
+    # test_disk_crossing_of_rays_through_the_axis_is_continuous_with_their_neighbours)
+    sc = W.scene(a, incl, 41, 18.0, ny=45)
+    thin = W.model_thin_disk(r_in=0.0, r_out=60.0)
+    out = ody.render_image(sc, thin); _sync()
+    gpu = {k: (_np(v) if v is not None else None) for k, v in out.items()}
+    ref = orc.render_image(sc, thin)
+    _check_disk(gpu, ref, check_hist=False)
+    col = ref["flag"].reshape(45, 41)[:, 20]
+    assert (col == W.FLAG_DISK).sum() >= 10 and col.max() <= 2
+    # hot spot: the azimuth of the crossing carries the k pi
+    mo = W.model_hot_spot(r_orbit=8.0, r_spot=2.0)
+    mo.update(r_in=0.0, r_out=60.0)
+    t_obs = [0.0, 40.0, 90.0]
+    hs = ody.render_hotspot(sc, mo, t_obs); _sync()
+    hr = orc.render_hotspot(sc, mo, t_obs)
+    assert np.array_equal(_np(hs["flag"]).ravel(), hr["flag"])
+    hit = hr["flag"] == W.FLAG_DISK
+    for key in ("g", "r_e", "phi_e", "t_e"):
+        x, xr = _np(hs[key]).ravel(), hr[key]
+        assert np.max(np.abs(x[hit] - xr[hit]) / np.maximum(np.abs(xr[hit]), 1.0)) <= 1e-8, key
+    for k in range(3):
+        if hr["images"][k].max() > 0:
+            assert np.abs(_np(hs["images"])[k].ravel() - hr["images"][k]).sum() / hr["images"][k].sum() <= 1e-6
+    # Novikov-Thorne disk on the same geometry
+    nt = W.model_nt_disk(r_out=60.0)
+    nu = [0.3 * KEV_HZ, 2.0 * KEV_HZ]
+    sp = ody.render_spectrum(sc, nt, nu); _sync()
+    sr = orc.render_spectrum(sc, nt, nu)
+    assert np.array_equal(_np(sp["flag"]).ravel(), sr["flag"])
+    for q in range(2):
+        _check_image(_np(sp["images"])[q].ravel(), sr["images"][q], "NT disk, centre column")

@@ -346,3 +346,33 @@ def test_the_two_transfer_schemes_converge_to_the_same_image():
         d.append(np.abs(a["image"] - b["image"]).sum() / a["image"].sum())
     assert d[0] > d[1] > d[2]
     assert d[2] < 2e-4
+
+
+# ------------------------------------------------------------------------------------------------
+# Rays through the rotation axis (L_z = 0: the centre column of an image with an odd number of columns) continue
+# with theta outside [0, pi]; they meet the equatorial plane at theta = pi/2 + k pi, the point (pi/2, phi + k pi).
+# Pin: continuity with their neighbours at x = +/- 1e-3, whose L_z != 0 keeps them inside (0, pi).
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("a, incl", [(0.0, 120.0), (0.0, 60.0), (0.9, 100.0), (0.998, 175.0)])
+def test_disk_crossing_of_rays_through_the_axis_is_continuous_with_their_neighbours(a, incl):
+    sc = W.scene(a, incl, 3, 12.0)
+    sc.update(ny=25, x_min=-1.5e-3, x_max=1.5e-3, y_min=-30.0, y_max=30.0)
+    mo = W.model_hot_spot(r_spot=1.0)
+    mo.update(r_in=0.0, r_out=60.0)
+    out = O.render_hotspot(sc, mo, [0.0])
+    flag = out["flag"].reshape(25, 3)
+    assert flag.max() <= 2                                      # nobody stuck (MAXSTEP) on the axis
+    r_e, g, phi = (out[k].reshape(25, 3) for k in ("r_e", "g", "phi_e"))
+    rows = np.nonzero((flag == 2).all(axis=1))[0]
+    assert len(rows) >= 12
+    through_axis = 0
+    for j in rows:
+        if abs(r_e[j, 0] - r_e[j, 2]) > 0.5:                    # a row where the two neighbours see different image orders
+            continue
+        assert r_e[j, 1] == pytest.approx(0.5 * (r_e[j, 0] + r_e[j, 2]), abs=2e-4)
+        assert g[j, 1] == pytest.approx(0.5 * (g[j, 0] + g[j, 2]), abs=2e-4)
+        # azimuth of the crossing point, modulo 2 pi: the neighbours swing round the axis by +pi and -pi
+        for k in (0, 2):
+            assert np.cos(phi[j, 1] - phi[j, k]) == pytest.approx(1.0, abs=1e-3)
+        through_axis += 1
+    assert through_axis >= 10
