@@ -140,9 +140,11 @@ int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model,
 /* nf <= 32 observed frequencies integrated simultaneously along each geodesic (kind 2 only;
  * BASELINE.json:configs[3]).  images[nf][ny][nx] = I_nu; nuLnu[nf] = 4π nu r_g^2 Δx Δy Σ_pixels I_nu
  * (erg/s; the distance cancels).  nu_hz_host is HOST memory.  rt_scheme must be ODYSSEY_RT_PER_STEP.
- * Images with fewer rays than four waves of resident lanes (~3e5 pixels on a B200) take a two-phase path
- * (record the geodesics once, then one lane per (ray, frequency)); that path synchronises `cuda_stream`
- * ONCE inside the call to read an overflow flag, and uses stream-ordered scratch (up to 28 KB per ray).
+ * Two code paths, same results to rounding: images of up to ~1.5e5 rays, and larger images with nf >= 12, take a
+ * two-phase path (record the geodesics once, then one lane per (ray, frequency); larger images band by band); it
+ * synchronises `cuda_stream` ONCE per band inside the call to read an overflow flag, and uses stream-ordered scratch
+ * (64 KB per ray of a band, ~10 GB at most).  Larger images with fewer frequencies take one fused kernel, no
+ * synchronisation.
  *
  * kind 4, the relativistic multi-temperature disk of Novikov & Thorne (eq. (35), Fig. 6): an
  * opaque disk on the equatorial plane between r_in (<= 0: r_isco) and r_out whose surface radiates as a blackbody

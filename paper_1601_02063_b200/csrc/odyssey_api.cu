@@ -147,6 +147,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
     P->r_h = 1.0 + std::sqrt(1.0 - S.a * S.a);
     P->r_cap = P->r_h + S.horizon_eps; P->r_esc = S.r_esc;
     P->nx = S.nx; P->ny = S.ny; P->max_attempts = S.max_attempts;
+    P->row0 = 0; P->ny_image = S.ny;
     P->tiles_x = (S.nx + TILE_W - 1) / TILE_W;
     const long long tiles_y = (S.ny + TILE_H - 1) / TILE_H;
     P->n_queue = (long long)P->tiles_x * tiles_y * (TILE_W * TILE_H);
@@ -304,13 +305,17 @@ int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
 
 Outputs no_outputs() { Outputs O; std::memset(&O, 0, sizeof(O)); return O; }
 
-// ---- two-phase spectrum path (small images; see spectrum_rt_kernel in odyssey_kernels.cuh) ------------------
-// Used when the image has fewer rays than TWO_PHASE_WAVES waves of resident lanes: there the fused spectrum
-// kernel's run time is the serial time of the longest ray.  Phases: record pass into fixed-capacity node lists,
-// ONE stream synchronisation to read its overflow flag (on overflow: count pass, prefix sum, exact-size record
-// pass), then the per-frequency transfer with one lane per (ray, frequency).
-constexpr int TWO_PHASE_WAVES = 4;
-constexpr long long NODE_CAP = 512;            // nodes per ray of the first, fixed-capacity attempt (28 KB per ray)
+// ---- two-phase spectrum path (see spectrum_rt_kernel in odyssey_kernels.cuh) -------------------------------
+// Phases: record pass into fixed-capacity node lists, ONE stream synchronisation to read its overflow flag (on
+// overflow: count pass, prefix sum, exact-size record pass), then the per-frequency transfer with one lane per
+// (ray, frequency).  It wins in two regimes: small images (fewer rays than a few waves of resident lanes, where the
+// fused spectrum kernel's run time is the serial time of the longest ray with all frequencies behind each other) and
+// many frequencies (the transfer kernel runs every lane on identical work: 1.5 ms per frequency and megaray
+// against 3.0 ms fused, for a fixed ~19 ms per megaray of recording).  Images larger than one band are processed
+// band by band (whole rows), so the node lists stay at ~10 GB whatever the image size.
+constexpr int TWO_PHASE_WAVES = 2;             // rays per band, in waves of the record kernel's resident lanes
+constexpr int TWO_PHASE_MIN_NF = 12;           // larger images with fewer frequencies take the fused kernel
+constexpr long long NODE_CAP = 1024;           // nodes per ray of the first, fixed-capacity attempt (64 KB per ray)
 
 template <int G>
 cudaError_t launch_spectrum_rt(const Params& P, const Outputs& O, int blocks, cudaStream_t st) {
@@ -318,7 +323,7 @@ cudaError_t launch_spectrum_rt(const Params& P, const Outputs& O, int blocks, cu
     return cudaGetLastError();
 }
 
-int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st) {
+int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st, bool zero_sed = true) {
     DevState* D = nullptr;
     TRY_RC(device_state(&D, nullptr));
     const size_t n = (size_t)P.nx * P.ny;
@@ -378,10 +383,10 @@ int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st) 
     }
     Outputs O2 = no_outputs();
     O2.images = user.images; O2.nuLnu = user.nuLnu; O2.flag = user.flag; O2.n_attempt = user.n_attempt;
-    O2.nodes = nodes; O2.node_offset = off; O2.node_cap = node_cap; O2.aux_nacc = iacc;
+    O2.nodes = nodes; O2.node_offset = off; O2.node_cap = node_cap; O2.aux_nacc = iacc; O2.image_stride = user.image_stride;
     O2.queue = next_counter(D);
     TP_TRY(cudaMemsetAsync(O2.queue, 0, sizeof(unsigned long long), st));
-    if (user.nuLnu) TP_TRY(cudaMemsetAsync(user.nuLnu, 0, sizeof(double) * P.nf, st));
+    if (user.nuLnu && zero_sed) TP_TRY(cudaMemsetAsync(user.nuLnu, 0, sizeof(double) * P.nf, st));
     if (user.flag) TP_TRY(cudaMemcpyAsync(user.flag, iflag, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
     if (user.n_attempt) TP_TRY(cudaMemcpyAsync(user.n_attempt, iatt, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
     O2.aux_flag = iflag;
@@ -495,9 +500,29 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
     rc = device_state(&D, nullptr);
     if (rc) return rc;
     const long long lanes = (long long)D->n_sm * 4 * NT_MAIN;                  // resident lanes of the record kernel
-    if ((long long)scene->nx * scene->ny <= TWO_PHASE_WAVES * lanes)
-        return render_spectrum_two_phase(P, O, scene->tableau, (cudaStream_t)cuda_stream);
-    return launch(P, O, true, scene->tableau, (cudaStream_t)cuda_stream);
+    const long long band_rays = TWO_PHASE_WAVES * lanes;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((long long)scene->nx * scene->ny <= band_rays)
+        return render_spectrum_two_phase(P, O, scene->tableau, st);
+    if (nf < TWO_PHASE_MIN_NF) return launch(P, O, true, scene->tableau, st);
+    // Larger images, many frequencies: the same two phases band by band (whole rows, about band_rays rays each);
+    // one stream synchronisation per band.
+    const int rows = (int)std::max<long long>(1, band_rays / scene->nx);
+    if (nuLnu) CUDA_TRY(cudaMemsetAsync(nuLnu, 0, sizeof(double) * nf, st));
+    for (int j0 = 0; j0 < scene->ny; j0 += rows) {
+        Params Pb = P;
+        Pb.ny = std::min(rows, scene->ny - j0); Pb.row0 = j0;
+        Pb.n_queue = (long long)Pb.tiles_x * ((Pb.ny + TILE_H - 1) / TILE_H) * (TILE_W * TILE_H);
+        Outputs Ob = O;
+        const size_t shift = (size_t)j0 * scene->nx;
+        if (images) Ob.images = images + shift;
+        if (flag) Ob.flag = flag + shift;
+        if (n_attempt) Ob.n_attempt = n_attempt + shift;
+        Ob.image_stride = (long long)scene->nx * scene->ny;
+        rc = render_spectrum_two_phase(Pb, Ob, scene->tableau, st, false);
+        if (rc) return rc;
+    }
+    return ODYSSEY_OK;
 }
 
 int odyssey_render_hotspot(const odyssey_scene* scene, const odyssey_model* model, const double* t_obs_host, int nt,

@@ -290,9 +290,9 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     *O.overflow = 1;                                       // the caller re-runs with exact sizes
                 } else {
                     const long long first = O.node_cap > 0 ? (long long)pix * O.node_cap : O.node_offset[pix];
-                    double* nd = O.nodes + NODE_DOUBLES * (first + slot);
-                    nd[0] = fresh ? 0.0 : h_try; nd[1] = pt.fac; nd[2] = pt.E; nd[3] = pt.t0; nd[4] = pt.u0; nd[5] = pt.ycoef;
-                    nd[6] = (double)n_att;
+                    double2* nd = reinterpret_cast<double2*>(O.nodes + NODE_DOUBLES * (first + slot));
+                    nd[0] = make_double2(fresh ? 0.0 : h_try, pt.fac); nd[1] = make_double2(pt.E, pt.t0);
+                    nd[2] = make_double2(pt.u0, pt.ycoef); nd[3] = make_double2((double)n_att, 0.0);
                 }
             }
         } else if (KIND == 2 && (commit || fresh)) {
@@ -476,6 +476,7 @@ __global__ void __launch_bounds__(128, 4) spectrum_rt_kernel(const __grid_consta
     const int lane = threadIdx.x & 31, k = lane % G, sub = lane / G;
     const unsigned gmask = (G == 32) ? FULL : (((1u << G) - 1u) << (sub * G));
     const int nf = P.nf, npix = P.nx * P.ny;
+    const size_t img_stride = O.image_stride ? (size_t)O.image_stride : (size_t)npix;
     const bool fk = k < nf;                                              // this lane owns a frequency
     Freq fq = freq_of(P, fk ? k : 0);                                    // lane-constant: fetched once (divergent constant loads)
     double nu3 = P.nu3[fk ? k : 0];
@@ -506,9 +507,9 @@ __global__ void __launch_bounds__(128, 4) spectrum_rt_kernel(const __grid_consta
         auto load_node = [&](int i, RtPoint& pt, double& h, double& natt) {
             pt.on = true;
             if (i < cnt) {
-                const double* nd = O.nodes + NODE_DOUBLES * (off + i);
-                h = __ldg(nd); pt.fac = __ldg(nd + 1); pt.E = __ldg(nd + 2); pt.t0 = __ldg(nd + 3); pt.u0 = __ldg(nd + 4);
-                pt.ycoef = __ldg(nd + 5); natt = __ldg(nd + 6);
+                const double2* nd = reinterpret_cast<const double2*>(O.nodes + NODE_DOUBLES * (off + i));
+                const double2 v0 = __ldg(nd), v1 = __ldg(nd + 1), v2 = __ldg(nd + 2), v3 = __ldg(nd + 3);
+                h = v0.x; pt.fac = v0.y; pt.E = v1.x; pt.t0 = v1.y; pt.u0 = v2.x; pt.ycoef = v2.y; natt = v3.x;
             } else { h = 0.0; natt = 0.0; pt.fac = 0.0; pt.E = 0.0; pt.t0 = 1.0; pt.u0 = 1.0; pt.ycoef = 0.0; }
         };
         RtPoint p0, p1, p2; double h0, h1, h2, n0, n1, n2;
@@ -531,7 +532,7 @@ __global__ void __launch_bounds__(128, 4) spectrum_rt_kernel(const __grid_consta
         }
         if (live && fk) {
             const double v = nu3 * I;
-            if (O.images) O.images[(size_t)k * npix + pix] = v;
+            if (O.images) O.images[(size_t)k * img_stride + pix] = v;
             if (O.nuLnu) atomicAdd(&sed[k], v);
         }
         if (live && k == 0 && opaque_att >= 0) {                         // the fused kernel's OPAQUE ending
@@ -553,7 +554,7 @@ __global__ void __launch_bounds__(256) init_rays_kernel(const __grid_constant__ 
         const int j = (tile / P.tiles_x) * TILE_H + (w / TILE_W);
         if (i >= P.nx || j >= P.ny) continue;                            // slot outside a ragged image: never read
         const double x = P.x_min + (i + 0.5) * P.x_span / P.nx;          // pixel centres (reading K)
-        const double yy = P.y_min + (j + 0.5) * P.y_span / P.ny;
+        const double yy = P.y_min + (j + P.row0 + 0.5) * P.y_span / P.ny_image;
         State y; double L;
         init_ray(P, x, yy, y, L);
         state[q] = y.r; state[q + P.n_queue] = y.th; state[q + 2 * P.n_queue] = y.ph;

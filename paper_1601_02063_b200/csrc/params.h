@@ -9,7 +9,8 @@ namespace ody {
 constexpr int MAX_FREQ = 32;
 constexpr int TILE_W = 8, TILE_H = 4;          // one queue tile = 8x4 pixels = one warp's first batch
 constexpr int LOCATE_MAX = 8;                  // Newton re-attempts of the event location
-constexpr int NODE_DOUBLES = 7;                // two-phase spectrum path: h, fac, E, t0, u0, ycoef, n_attempt per node
+constexpr int NODE_DOUBLES = 8;                // two-phase spectrum path: h, fac, E, t0, u0, ycoef, n_attempt (+ 1 pad) per node:
+                                               // 64 bytes, written and read as four aligned 16-byte vectors (two whole 32-byte sectors)
 
 struct Params {
     // ---- scene
@@ -40,6 +41,7 @@ struct Params {
     double sed_coef;                            // 4π r_g^2 Δx Δy
     int32_t nf, rt_scheme;                      // rt_scheme: ODYSSEY_RT_* (kind 2); internally 2 = record pass, 3 = per-step with the Δτ cap
     double dtau_max;                            // (rt_scheme 3) cap of the next step's optical depth
+    int32_t row0, ny_image;                     // this launch covers image rows [row0, row0 + ny) of ny_image (bands of the two-phase spectrum path)
     int32_t precision, pad3;                    // ODYSSEY_PREC_* (kind 2)
     // ---- hot spot (kind 3; eq. (36)); the observer times t_obs[k] travel in nu[k], nf = their number
     double spot_R, spot_Omega, spot_phi0;       // sqrt(r_s² + a²), 1/(r_s^{3/2} + a), azimuth at t = 0
@@ -73,6 +75,7 @@ struct Outputs {
     int32_t* overflow;                           // record pass: set to 1 when a ray needs more than node_cap nodes
     unsigned long long* queue;                   // work-queue counter (zeroed before the launch)
     const double* init_state;                    // library scratch: initial states by queue slot, [6][n_queue] (init_rays_kernel)
+    long long image_stride;                      // spectrum_rt_kernel: elements between the images of two frequencies (0: nx * ny)
 };
 
 }  // namespace ody
