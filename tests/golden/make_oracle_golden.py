@@ -39,6 +39,18 @@ def main():
                             "phi_e": hs["phi_e"].tolist(), "images": hs["images"].tolist()}
     g = O.trace_geodesics(W.C0(n=8)["scene"])
     out["C0_8x8"]["t"] = g["t"].tolist()
+    # Novikov-Thorne disk (reading NT): f(r), T_eff and a small spectrum of Fig. 6's set-up
+    nt = W.model_nt_disk()
+    out["nt_disk"] = {"a": 0.999, "r": [1.3, 2.0, 6.0, 30.0],
+                      "f": [O.page_thorne_f(0.999, r) for r in (1.3, 2.0, 6.0, 30.0)],
+                      "T_eff": [O.nt_temperature(nt, 0.999, r) for r in (1.3, 2.0, 6.0, 30.0)]}
+    nu_nt = [2.4e16, 2.4e17, 1.2e18]
+    sp = O.render_spectrum(W.scene(0.999, 85.0, 9, 25.0), nt, nu_nt)
+    out["nt_disk"].update(nu=nu_nt, nuLnu=sp["nuLnu"].tolist(), images=sp["images"].tolist(), flag=sp["flag"].tolist())
+    # optical-depth step cap (reading DT) on the optically thick 10 GHz image
+    w = W.C2(n=8)
+    r = O.render_image(w["scene"], W.model_riaf(dtau_max=0.1), 1.0e10)
+    out["C2_8x8_10GHz_dtau0.1"] = {"image": r["image"].tolist(), "tau": r["aux0"].tolist(), "n_attempt": r["n_attempt"].tolist()}
     with open(os.path.join(HERE, "oracle_regression.json"), "w") as f:
         json.dump(out, f, indent=1)
     print("wrote oracle_regression.json")

@@ -97,6 +97,15 @@ def test_oracle_regression_values():
     w = W.C3(n=4, nf=4)
     s = O.render_spectrum(w["scene"], w["model"], w["nu"])
     _cmp(s["nuLnu"], ORACLE["C3_4x4_nf4"]["nuLnu"], 1e-10)
+    nt = ORACLE["nt_disk"]
+    _cmp([O.page_thorne_f(nt["a"], r) for r in nt["r"]], nt["f"], 1e-12)
+    _cmp([O.nt_temperature(W.model_nt_disk(), nt["a"], r) for r in nt["r"]], nt["T_eff"], 1e-12)
+    sp = O.render_spectrum(W.scene(0.999, 85.0, 9, 25.0), W.model_nt_disk(), nt["nu"])
+    assert sp["flag"].tolist() == nt["flag"]
+    _cmp(sp["nuLnu"], nt["nuLnu"], 1e-9)
+    r = O.render_image(W.C2(n=8)["scene"], W.model_riaf(dtau_max=0.1), 1.0e10)
+    assert r["n_attempt"].tolist() == ORACLE["C2_8x8_10GHz_dtau0.1"]["n_attempt"]
+    _cmp(r["image"], ORACLE["C2_8x8_10GHz_dtau0.1"]["image"], 1e-10)
 
 
 @pytest.mark.gpu
@@ -120,3 +129,10 @@ def test_cuda_path_against_stored_oracle_values(ody):
     w = W.C3(n=4, nf=4)
     s = ody.render_spectrum(w["scene"], w["model"], w["nu"]); torch.cuda.synchronize()
     _cmp(s["nuLnu"].cpu().numpy(), ORACLE["C3_4x4_nf4"]["nuLnu"], 1e-6)
+    nt = ORACLE["nt_disk"]
+    sp = ody.render_spectrum(W.scene(0.999, 85.0, 9, 25.0), W.model_nt_disk(), nt["nu"]); torch.cuda.synchronize()
+    assert sp["flag"].cpu().numpy().ravel().tolist() == nt["flag"]
+    _cmp(sp["nuLnu"].cpu().numpy(), nt["nuLnu"], 1e-6)
+    r = ody.render_image(W.C2(n=8)["scene"], W.model_riaf(dtau_max=0.1), 1.0e10); torch.cuda.synchronize()
+    img, st = r["image"].cpu().numpy().ravel(), np.asarray(ORACLE["C2_8x8_10GHz_dtau0.1"]["image"])
+    assert np.abs(img - st).sum() / st.sum() <= 1e-6
