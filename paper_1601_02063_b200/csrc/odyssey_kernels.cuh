@@ -517,6 +517,9 @@ __global__ void __launch_bounds__(128, 4) spectrum_rt_kernel(const __grid_consta
         double a_prev, e_prev, a_cur, e_cur;
         rt_coefficients<true>(P, p0, fq, a_prev, e_prev);                // node 0: start point
         rt_coefficients<true>(P, p1, fq, a_cur, e_cur);                  // node 1
+        // (one ray per warp: two trips per iteration give the scheduler a third independent chain, -4 %; with several
+        // rays of different lengths per warp the unrolled loop loses more on its tail than it gains)
+#pragma unroll (G == 32 ? 2 : 1)
         for (int i = 1; i < cmax; ++i) {
             RtPoint p3; double h3, n3;
             load_node(i + 2, p3, h3, n3);                                // two ahead
