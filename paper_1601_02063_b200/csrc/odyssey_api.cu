@@ -504,7 +504,7 @@ int odyssey_render_spectrum(const odyssey_scene* scene, const odyssey_model* mod
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if ((long long)scene->nx * scene->ny <= band_rays)
         return render_spectrum_two_phase(P, O, scene->tableau, st);
-    if (nf < TWO_PHASE_MIN_NF) return launch(P, O, true, scene->tableau, st);
+    if (nf < TWO_PHASE_MIN_NF || scene->nx > band_rays) return launch(P, O, true, scene->tableau, st);   // (bands are whole rows)
     // Larger images, many frequencies: the same two phases band by band (whole rows, about band_rays rays each);
     // one stream synchronisation per band.
     const int rows = (int)std::max<long long>(1, band_rays / scene->nx);
