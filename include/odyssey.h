@@ -31,6 +31,9 @@
  *     the device's default stream-ordered memory pool (cudaMallocAsync / cudaFreeAsync on `cuda_stream`).
  *   - Every call first runs a camera kernel (initial conditions of all pixels), then the persistent
  *     integrator kernel: two kernel launches of this library per call (more in spectrum mode).
+ *   - All of that is stream-ordered, so a DEVICE call may be captured into a CUDA graph and replayed (the captured
+ *     graph keeps the call's queue counter: replay it on one stream at a time).  The exception is the two-phase path
+ *     of odyssey_render_spectrum, which synchronises the stream inside the call.
  */
 #ifndef ODYSSEY_H_
 #define ODYSSEY_H_

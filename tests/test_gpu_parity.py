@@ -257,3 +257,23 @@ def test_maximum_image_size_two_to_the_thirty_pixels(ody, orc):
     assert np.max(np.abs(r[jj, ii].cpu().numpy() - ref["r"]) / ref["r"]) <= 1e-8
     del flag, natt, r
     torch.cuda.empty_cache()
+
+
+def test_image_call_can_be_captured_in_a_cuda_graph(ody):
+    # every step of odyssey_render_image is stream-ordered (scratch from cudaMallocAsync, memsets, two kernels, no
+    # synchronisation), so the call can be captured once and replayed
+    import torch
+    w = W.C2(n=64)
+    out = ody.render_image(w["scene"], w["model"], w["nu"][0]); _sync()
+    ref, ref_att = out["image"].clone(), out["n_attempt"].clone()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        ody.render_image(w["scene"], w["model"], w["nu"][0], out=out)
+    _sync()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        ody.render_image(w["scene"], w["model"], w["nu"][0], out=out)
+    for _ in range(3):
+        out["image"].zero_(); out["n_attempt"].zero_()
+        graph.replay(); _sync()
+        assert bool((out["image"] == ref).all()) and bool((out["n_attempt"] == ref_att).all())
