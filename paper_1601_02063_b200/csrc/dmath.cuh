@@ -160,7 +160,7 @@ ODY_HD void d_sincos(double x, double& sn, double& cs) {
 #endif
     for (int i = ODY_SINS_N - 2; i >= 0; --i) { ps = d_fma(ps, z, S[i]); pc = d_fma(pc, z, C[i]); }
     const double sr = d_fma(ps * z, r, r);                         // r + r^3 S(z)
-    const double cr = d_fma(z * z, pc, d_fma(-0.5, z, 1.0));       // 1 - z/2 + z^2 C(z)
+    const double cr = d_fma(z, d_fma(z, pc, -0.5), 1.0);           // 1 - z/2 + z^2 C(z), Horner: both constants are 32-bit immediates
     const bool swap = q & 1;
     const double s0 = swap ? cr : sr, c0 = swap ? sr : cr;
     sn = d_xor_sign(s0, (uint32_t)q << 30);                        // negative in quadrants 2, 3

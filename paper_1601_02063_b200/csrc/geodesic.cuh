@@ -23,6 +23,16 @@ struct Slope { double r, th, ph, pr, pth, t; };  // dy/dλ; t (eq. (9)) is forme
 // ------------------------------------------------------------------------------------------------
 // Right-hand side.  Also returns sinθ, cosθ (unclamped) for the emission code.
 // ------------------------------------------------------------------------------------------------
+// The pole clamp of PAPER.md:L90 (reading I): |sinθ| < 1e-8 -> copysign(1e-8, sinθ).  The comparison is made on the
+// bit patterns (for finite doubles |x| < |y| <=> bits(|x|) < bits(|y|) as integers): two integer compares and
+// three selects on the ALU pipe instead of a DSETP, which would take an FP64-pipe slot in every right-hand side.
+__device__ __forceinline__ double clamp_sin(const double s) {
+    const int hi = __double2hiint(s), lo = __double2loint(s);
+    const unsigned long long mag = ((unsigned long long)(unsigned)(hi & 0x7fffffff) << 32) | (unsigned)lo;
+    const bool small = mag < 0x3E45798EE2308C3Aull;                // bits(1e-8)
+    return small ? __hiloint2double((hi & 0x80000000) | 0x3E45798E, (int)0xE2308C3A) : s;
+}
+
 template <bool TIME = false>
 __device__ __forceinline__ void geodesic_rhs(const double a, const double a2, const double L,
                                              const double r, const double th, const double pr, const double pth,
@@ -30,7 +40,7 @@ __device__ __forceinline__ void geodesic_rhs(const double a, const double a2, co
     double s, c;
     d_sincos(th, s, c);
     sin_th = s; cos_th = c;
-    if (fabs(s) < 1e-8) s = copysign(1e-8, s);
+    s = clamp_sin(s);
     // 37 FP64 operations + three reciprocals (was 43): shared sub-expressions r² + a², 2q + G/Σ
     const double r2 = r * r;
     const double ra2 = r2 + a2;                                   // r² + a²
@@ -187,47 +197,41 @@ __device__ __forceinline__ void rk_combine(const KS& K, const State& y, const do
 }
 
 // Scaled max-norm of the error in units of rtol (reading G): scales (|r|, 1, 1, 1+|p_r|,
-// 1+|p_θ|).  A NaN anywhere yields NaN (the attempt is then rejected with h × 0.1).
+// 1+|p_θ|).  The maximum is taken on the BIT PATTERNS of the five non-negative quotients: for non-negative doubles
+// the integer order is the floating-point order, +inf sorts above every finite value and a NaN (0x7ff8…, sign
+// cleared) above +inf, so a NaN anywhere comes out as NaN (the attempt is then rejected with h × 0.1) without a
+// separate test — and the compares run on the ALU pipe, not on the FP64 pipe.  r > r_h > 0 on every live ray.
+__device__ __forceinline__ long long abs_bits(const double x) { return __double_as_longlong(x) & 0x7fffffffffffffffLL; }
 __device__ __forceinline__ double error_norm(const State& y, const State& e, const double inv_rtol) {
-    const double q0 = fabs(e.r) * d_rcp(fabs(y.r));
-    const double q1 = fabs(e.th), q2 = fabs(e.ph);
-    const double q3 = fabs(e.pr) * d_rcp(1.0 + fabs(y.pr));
-    const double q4 = fabs(e.pth) * d_rcp(1.0 + fabs(y.pth));
-    // plain compare-and-select maxima (fmax's NaN rules cost a dozen instructions each); NaNs are caught below
-    double m = q0 > q1 ? q0 : q1;
-    const double m2 = q2 > q3 ? q2 : q3;
-    m = m > m2 ? m : m2;
-    m = m > q4 ? m : q4;
-    const double sum = q0 + q1 + q2 + q3 + q4;                     // NaN anywhere -> NaN here (all q >= 0)
-    return (sum != sum) ? sum : m * inv_rtol;
+    const long long b0 = abs_bits(e.r * d_rcp(y.r));
+    const long long b1 = abs_bits(e.th), b2 = abs_bits(e.ph);
+    const long long b3 = abs_bits(e.pr * d_rcp(1.0 + fabs(y.pr)));
+    const long long b4 = abs_bits(e.pth * d_rcp(1.0 + fabs(y.pth)));
+    const long long m01 = b0 > b1 ? b0 : b1, m23 = b2 > b3 ? b2 : b3;
+    const long long m = m01 > m23 ? m01 : m23;
+    return __longlong_as_double(m > b4 ? m : b4) * inv_rtol;
 }
 
-// x^(-1/5) for x in (0, 1]: MUFU.LG2 / MUFU.EX2 seed in single precision (relative error ~1e-6), two
-// Newton steps y <- y (6 - x y^5)/5 in FP64 (error -> 3e^2 per step).
-__device__ __forceinline__ double inv_fifth_root(const double x) {
+// Step-size factor of the controller (reading G), one straight-line evaluation for both outcomes:
+//   accepted attempt: min(5, 0.9 err^-1/5)  (5 below err = 1.889568e-4),   rejected: max(0.1, 0.9 err^-1/4).
+// y = err^-1/n from a single-precision seed (MUFU.LG2 / MUFU.EX2, relative error d ~ 1e-6) and ONE third-order
+// step y (1 + e/n + (n+1) e^2 / (2 n^2)), e = 1 - err y^n = -n d, which leaves (n+1)(2n+1)/(6 n^3) e^3 < 2e-17:
+// the factor is correct to the rounding of its last operations.  Out-of-range arguments need no test: err = 0
+// or denormal gives y = inf or NaN and the clamp returns 5; err = inf, NaN or > 1e38 gives 0 or NaN -> 0.1.
+// (The first version branched: the two bodies ran one after the other in nearly every trip, the rejected one
+// 6 lanes wide, and each was a serial chain of ~14 FP64 operations.)
+__device__ __forceinline__ double step_factor(const double err, const bool accepted) {
     float l, sd;
-    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"((float)x));
-    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(sd) : "f"(-0.2f * l));
-    double y = (double)sd;
-#pragma unroll
-    for (int it = 0; it < 2; ++it) {
-        const double y2 = y * y;
-        const double y5 = y2 * y2 * y;
-        y = y * fma(-x, y5, 6.0) * 0.2;
-    }
-    return y;
-}
-
-// Step-size factors of the controller (reading G), with compare-and-select clamps.
-__device__ __forceinline__ double grow_factor(const double err) {          // accepted: min(5, 0.9 err^-0.2)
-    if (err < 1.889568e-4) return 5.0;
-    const double f = 0.9 * inv_fifth_root(err);
-    return f < 5.0 ? f : 5.0;
-}
-__device__ __forceinline__ double shrink_factor(const double err) {        // rejected: max(0.1, 0.9 err^-0.25)
-    if (!(err < 1e300)) return 0.1;                                        // infinite or NaN
-    const double f = 0.9 * d_rsqrt(d_sqrt(err));
-    return f > 0.1 ? f : 0.1;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"((float)err));
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(sd) : "f"((accepted ? -0.2f : -0.25f) * l));
+    const double y = (double)sd;
+    const double y2 = y * y, y4 = y2 * y2;
+    const double yn = accepted ? y4 * y : y4;
+    const double e = fma(-err, yn, 1.0);
+    const double p = fma(e, accepted ? 0.12 : 0.15625, accepted ? 0.2 : 0.25);
+    const double f = 0.9 * fma(y * e, p, y);
+    const double lim = accepted ? 5.0 : 0.1;
+    return accepted ? (f < lim ? f : lim) : (f > lim ? f : lim);   // a NaN takes the limit in both cases
 }
 
 // ------------------------------------------------------------------------------------------------

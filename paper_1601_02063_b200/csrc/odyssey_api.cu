@@ -215,7 +215,10 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
 }
 
 // ---- kernel table ------------------------------------------------------------------------------
-constexpr int NT_MAIN = 128, MINB_MAIN = 5;     // 96 registers per thread at most
+#ifndef ODY_MINB_MAIN
+#define ODY_MINB_MAIN 5
+#endif
+constexpr int NT_MAIN = 128, MINB_MAIN = ODY_MINB_MAIN;     // 96 registers per thread at most
 constexpr int MINB_SPOT = 4;                    // hot spot (kind 3, with the coordinate time) and Novikov-Thorne disk (kind 4): 4 blocks per SM keep them free of spills
 constexpr int MINB_RK = 2;                      // transfer scheme E' (RK components): the in-loop transfer code wants > 168 registers
 constexpr int NT_SPEC = 128, MINB_SPEC = 3;     // 168 registers (the unrolled frequency loop wants them); per-frequency accumulators in a global scratch buffer

@@ -164,7 +164,11 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         double ir, ith, ipr, ipth, yn_ph = y.ph;
         Slope k; double sn, cn;
 
-#pragma unroll 1
+#ifndef ODY_STAGE_UNROLL
+#define ODY_STAGE_UNROLL 6
+#endif
+        constexpr int kStageUnroll = ODY_STAGE_UNROLL;
+#pragma unroll kStageUnroll
         for (int s = 1; s <= 6; ++s) {
             bool ev = run;
             switch (s) {
@@ -180,13 +184,10 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                         ++n_att;
                         if (mode == M_NORMAL) {
                             const double err = error_norm(y, ye, P.inv_rtol);
-                            if (!(err <= 1.0)) {                       // reject (also NaN): shrink, keep k1
-                                h_try *= shrink_factor(err);
-                                ev = false;
-                            } else {
-                                ++n_acc;
-                                h_next = h_try * grow_factor(err);
-                            }
+                            const bool accepted = err <= 1.0;          // a NaN is rejected
+                            const double hf = h_try * step_factor(err, accepted);
+                            if (accepted) { ++n_acc; h_next = hf; }
+                            else { h_try = hf; ev = false; }           // shrink, keep k1
                         } else {
                             ++loc_it;
                         }
@@ -198,7 +199,13 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     done = ev;
                 }
             }
+#ifndef ODY_COND_STAGES
+            // stages 1..5 run for every lane: a lane without a running attempt (fresh, idle) computes values nobody reads
+            // (its slopes are rewritten before they are used), and the five stages form one straight-line block
+            if (s < 6 || ev) {
+#else
             if (ev) {
+#endif
                 geodesic_rhs<TIME != 0>(a, a2, L, ir, ith, ipr, ipth, k, sn, cn);
                 if (TIME && s < 6) {
                     const double b5s = (s == 1) ? kRkB5[TAB][1] : (s == 2) ? kRkB5[TAB][2] : (s == 3) ? kRkB5[TAB][3]

@@ -122,7 +122,13 @@ def test_spectrum_matches_single_frequency_calls(ody):
     for k, nu in enumerate(w["nu"]):
         one = ody.render_image(w["scene"], w["model"], nu); _sync()
         a, b = _np(spec["images"][k]), _np(one["image"])
-        assert np.allclose(a, b, rtol=1e-12, atol=0.0)
+        # The two kernels form x_M^(1/12) in a different order (spectrum: (x_M/nu)^(1/12) * nu^(1/12), image: one
+        # exponential), and eq. (38)'s exponent -1.8899 x_M^(1/3) reaches -550 at 1e15 Hz (pixel values ~1e-240):
+        # a rounding difference of one ulp in x_M^(1/12) is 4 * 550 ulp = 2.4e-13 in such a pixel, per point of
+        # the ray.  1e-12 holds wherever the value is above 1e-100; the deep-underflow pixels get 1e-11.
+        big = np.abs(b) >= 1e-100
+        assert np.allclose(a[big], b[big], rtol=1e-12, atol=0.0)
+        assert np.allclose(a[~big], b[~big], rtol=1e-11, atol=0.0)
 
 
 def test_c3_full_size_sampled(ody, orc):
