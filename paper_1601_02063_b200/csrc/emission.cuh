@@ -205,6 +205,27 @@ __device__ __forceinline__ void rt_update(const double a0, const double a1, cons
     tau = live ? tau + dtau : tau;
 }
 
+// The same update in two parts, for the transfer FIFO of the single-frequency kernel: what depends only on the
+// coefficients at the two ends of the step (the expensive part: an exponential and a reciprocal), and the
+// recurrence in tau, T, I.  Operation for operation the arithmetic of rt_update().
+template <int PREC = 0>
+__device__ __forceinline__ void rt_increments(const double a0, const double a1, const double e0, const double e1, const double dl,
+                                              double& dtau, double& em, double& phi, double& w) {
+    dtau = 0.5 * (a0 + a1) * dl;
+    em = p_expm1_nc<PREC>(dtau < 700.0 ? -dtau : -700.0);
+    phi = (dtau > 1e-300) ? -em * d_rcp(dtau) : 1.0;
+    w = 0.5 * (e0 + e1) * dl;
+}
+__device__ __forceinline__ void rt_accumulate(const double dtau, const double em, const double phi, const double w,
+                                              const double tau_max, double& tau, double& T, double& I) {
+    const bool live = !(tau > tau_max);
+    const double In = fma(T * w, phi, I);
+    const double Tn = fma(T, em, T);
+    I = live ? In : I;
+    T = live ? Tn : T;
+    tau = live ? tau + dtau : tau;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Novikov–Thorne disk (kind 4; eq. (35); reading NT): effective temperature at radius r,
 // σ T_eff⁴ = 3 Mdot M f(r)/(8π r³) with Page & Thorne's closed form of f for zero torque at r_isco,

@@ -139,11 +139,12 @@ __constant__ double kRkBE[2][6] = { ODY_BE(0), ODY_BE(1) };
 // words, so every access is conflict-free.  This takes 48 registers off the kernel, which is what lets
 // it run 5 blocks of 128 threads per SM at 96 registers without spills.
 constexpr int STAGE_ROWS = 5;                           // r, θ, p_r, p_θ slopes + the absorption coefficient (RT scheme E')
+constexpr int STAGE_SLOTS = 5;                          // k1..k5 are stored; the sixth slope goes from registers straight into the result
 template <int NT>
 struct StagesSmem {
     double* base;                                       // &smem[threadIdx.x]
-    __device__ __forceinline__ double get(int c, int j) const { return base[(c * 6 + j) * NT]; }
-    __device__ __forceinline__ void set(int c, int j, double x) { base[(c * 6 + j) * NT] = x; }
+    __device__ __forceinline__ double get(int c, int j) const { return base[(c * STAGE_SLOTS + j) * NT]; }
+    __device__ __forceinline__ void set(int c, int j, double x) { base[(c * STAGE_SLOTS + j) * NT] = x; }
 };
 
 // Argument of stage I+1 (0-based I in 1..5): y + h Σ_{j<I} a_Ij k_j.
@@ -175,9 +176,10 @@ __device__ __forceinline__ double stage_sum(const KS& K, const int c) {
 // Fifth-order result and the error estimate h Σ (b5_j − b4_j) k_j (as Press et al.'s rkck forms it)
 // of the four dynamic components; ph5 / phe are the kernel's running φ sums.
 template <int TAB, class KS>
-__device__ __forceinline__ void rk_combine(const KS& K, const State& y, const double h, const double ph5, const double phe,
+__device__ __forceinline__ void rk_combine(const KS& K, const Slope& k6, const State& y, const double h, const double ph5, const double phe,
                                            State& ynew, State& yerr) {
     double s5[4] = {0.0, 0.0, 0.0, 0.0}, se[4] = {0.0, 0.0, 0.0, 0.0};
+    const double last[4] = {k6.r, k6.th, k6.pr, k6.pth};
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
         const bool has5 = rk_b5<TAB>(j) != 0.0, hase = (rk_b5<TAB>(j) - rk_b4<TAB>(j)) != 0.0;
@@ -185,7 +187,7 @@ __device__ __forceinline__ void rk_combine(const KS& K, const State& y, const do
             const double b5 = kRkB5[TAB][j], be = kRkBE[TAB][j];
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                const double k = K.get(c, j);
+                const double k = (j < 5) ? K.get(c, j) : last[c];
                 if (has5) s5[c] = fma(b5, k, s5[c]);
                 if (hase) se[c] = fma(be, k, se[c]);
             }

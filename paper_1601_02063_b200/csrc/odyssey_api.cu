@@ -253,6 +253,7 @@ size_t smem_bytes(int kind, bool spec, int nf, int nbins, int rts = 0) {
     const size_t stages = (size_t)smem_per_thread(kind == 2 ? rts : 0) * NT_MAIN * sizeof(double);   // stage values + [5][NT] RT state
     if (kind == 1) return stages + (size_t)(nbins > 0 ? nbins : 1) * sizeof(double);
     if (kind == 4) return stages + (size_t)MAX_FREQ * sizeof(double);
+    if (uses_fifo(kind, spec, rts)) return stages + (size_t)fifo_doubles_per_block(NT_MAIN) * sizeof(double);
     return stages;
 }
 

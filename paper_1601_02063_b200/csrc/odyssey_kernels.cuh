@@ -49,14 +49,26 @@ __device__ __forceinline__ int radial_event(const Params& P, const State& yn) {
 
 template <int TAB, int I, class KS>
 __device__ __forceinline__ void store_stage(KS& K, const Slope& k, double& ph5, double& phe) {
-    K.set(0, I, k.r); K.set(1, I, k.th); K.set(2, I, k.pr); K.set(3, I, k.pth);
+    if (I < STAGE_SLOTS) { K.set(0, I, k.r); K.set(1, I, k.th); K.set(2, I, k.pr); K.set(3, I, k.pth); }
     if (rk_b5<TAB>(I) != 0.0) ph5 = fma(kRkB5[TAB][I], k.ph, ph5);
     if (rk_b5<TAB>(I) - rk_b4<TAB>(I) != 0.0) phe = fma(kRkBE[TAB][I], k.ph, phe);
 }
 
-// Shared-memory doubles per thread: rows x 6 stage values + 5 single-frequency transfer values
+// Shared-memory doubles per thread: rows x 5 stored stage values + 5 single-frequency transfer values
 // (rows = 4 slopes, + the absorption coefficient for transfer scheme E').
-__host__ __device__ constexpr int smem_per_thread(int rts) { return (rts == 1 ? STAGE_ROWS : STAGE_ROWS - 1) * 6 + 5; }
+__host__ __device__ constexpr int smem_per_thread(int rts) { return (rts == 1 ? STAGE_ROWS : STAGE_ROWS - 1) * STAGE_SLOTS + 5; }
+
+// Transfer FIFO (single-frequency per-step scheme): per warp a ring of FIFO_CAP points waiting for their
+// absorption / emission coefficients — 5 doubles (r, sinθ, cosθ, p_r, step length) and 4 ints (owner lane | flags,
+// position of the owner's previous point, attempted and accepted step counts) each — plus, per thread, the ray's L
+// and the step counts at which the ray turned opaque.
+#ifndef ODY_RT_FIFO
+#define ODY_RT_FIFO 1
+#endif
+constexpr int FIFO_CAP = 64;
+constexpr int FIFO_DOUBLES = 7 * FIFO_CAP;                               // per warp
+__host__ __device__ constexpr bool uses_fifo(int kind, bool spec, int rts) { return ODY_RT_FIFO && kind == 2 && !spec && rts == 0; }
+__host__ __device__ constexpr int fifo_doubles_per_block(int nt) { return nt + (nt / 32) * FIFO_DOUBLES + nt; }   // L, rings, 2 ints per thread
 
 // RTS = 1: transfer scheme E' (tau, I as Runge–Kutta components; single frequency only).
 // RTS = 2: record mode, the first phase of the two-phase spectrum path (see spectrum_rt_kernel below).
@@ -70,7 +82,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     constexpr bool HAS_EQ = (KIND == 1 || KIND == 3 || KIND == 4);     // models on the equatorial plane
     const int lane = threadIdx.x & 31;
     const int nf = SPEC ? P.nf : 1;
-    // shared layout: [5][6][NT] stage values, [5][NT] single-frequency RT state, then hist[nbins] (KIND 1)
+    // shared layout: [rows][5][NT] stage values, [5][NT] single-frequency RT state, then hist[nbins] (KIND 1)
     // or sed[MAX_FREQ] (SPEC).  The spectrum variant's 5 x nf per-frequency accumulators live in a global
     // scratch buffer laid out [quantity][frequency][grid thread] (every warp access is one contiguous
     // 256-byte segment; 160 doubles per thread would cap the SM at 5 warps if they sat in shared memory).
@@ -85,6 +97,19 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     if (SPEC || KIND == 1 || KIND == 4) __syncthreads();
 #define ACC(q, k) gl_acc[((q) * nf + (k)) * spec_stride]            // q: 0 tau, 1 T, 2 I, 3 a0, 4 e0
 
+    // Transfer FIFO (see the transfer section of the loop)
+    constexpr bool FIFO = uses_fifo(KIND, SPEC, RTS);
+    double* const sm_L = sm_red;                                                          // [NT] L of the lane's ray
+    double* const sm_ring = sm_red + NT + (threadIdx.x >> 5) * FIFO_DOUBLES;              // this warp's ring
+    int* const sm_ringi = reinterpret_cast<int*>(sm_ring + 5 * FIFO_CAP);
+    int* const sm_opq = reinterpret_cast<int*>(sm_red + NT + (NT / 32) * FIFO_DOUBLES);   // [2][NT]: n_attempt, n_accept at the opaque crossing
+    double* const sm_rtw = smem + (smem_per_thread(RTS) - 5) * NT + (threadIdx.x & ~31);  // RT state of this warp's lane 0
+#define FD(f, slot) sm_ring[(f) * FIFO_CAP + (slot)]
+#define FI(g, slot) sm_ringi[(g) * FIFO_CAP + (slot)]
+    unsigned f_head = 0, f_tail = 0, my_last = 0u - 1u;                                   // ring positions (warp-uniform head, tail)
+    int drain_wait = 0, end_flag = -1;
+    bool draining = false, prev_out = true;
+
     const double a = P.a, a2 = P.a2;
     bool active = false, exhausted = false, on_eq = false;
     int pix = 0, n_att = 0, n_acc = 0, mode = M_NORMAL, loc_it = 0;
@@ -97,17 +122,85 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     double g_disk = 0.0, r_e = 0.0;
     y.r = y.th = y.ph = y.pr = y.pth = 0.0;
 #pragma unroll
-    for (int j = 0; j < 6; ++j) { K.set(0, j, 0.0); K.set(1, j, 0.0); K.set(2, j, 0.0); K.set(3, j, 0.0); }
+    for (int j = 0; j < STAGE_SLOTS; ++j) { K.set(0, j, 0.0); K.set(1, j, 0.0); K.set(2, j, 0.0); K.set(3, j, 0.0); }
+
+    // ---- transfer FIFO: one batch of up to 32 waiting points, one point per lane whoever owns it (see the transfer
+    // section of the loop).  Phase A — coefficients at the point (the expensive part, every lane busy); phase B — the
+    // step's optical depth, attenuation and emission from the coefficients at its two ends (the start values are the
+    // previous point's: in this batch, or in the owner's state); phase C — the recurrence in tau, T, I of eqs. (30),
+    // (31), in the order of the steps: a point waits until its owner's previous point in the batch is done.
+    // Arithmetic and order per ray are those of rt_update(): the results do not depend on the batching.
+    auto fifo_process = [&]() {
+        const int cnt = (int)(f_tail - f_head);
+        const int nb = cnt < 32 ? cnt : 32;
+        const bool have = lane < nb;
+        const int slot = (int)((f_head + lane) & (FIFO_CAP - 1));
+        double er = 0.0, esn = 0.0, ecn = 0.0, epr = 0.0, eh = 0.0;
+        int meta = 0, prevpos = 0, eatt = 0, eacc = 0;
+        if (have) {
+            er = FD(0, slot); esn = FD(1, slot); ecn = FD(2, slot); epr = FD(3, slot); eh = FD(4, slot);
+            meta = FI(0, slot); prevpos = FI(1, slot); eatt = FI(2, slot); eacc = FI(3, slot);
+        }
+        const int o = meta & 31;
+        double a1 = 0.0, e1 = 0.0;
+        if (have) {
+            RtPoint pt; rt_point<false, PREC>(P, sm_L[(threadIdx.x & ~31) + o], er, esn, ecn, epr, pt);
+            rt_coefficients<false, PREC>(P, pt, freq_of(P, 0), a1, e1);
+            FD(0, slot) = a1; FD(1, slot) = e1;
+        }
+        __syncwarp();
+        const int pd = (int)((unsigned)prevpos - f_head);            // >= 0: the owner's previous point is in this batch
+        double* const st = sm_rtw + o;                                // the owner's tau, T, I, a0, e0
+        double dtau = 0.0, em = 0.0, phi = 1.0, w = 0.0;
+        if (have) {
+            double a0, e0;
+            if (pd >= 0) { const int ps = prevpos & (FIFO_CAP - 1); a0 = FD(0, ps); e0 = FD(1, ps); }
+            else { a0 = st[3 * NT]; e0 = st[4 * NT]; }
+            rt_increments<PREC>(a0, a1, e0, e1, eh, dtau, em, phi, w);
+        }
+        bool mine = !have;
+        for (;;) {
+            const unsigned dm = __ballot_sync(FULL, mine);
+            if (dm == FULL) break;
+            if (!mine && (pd < 0 || ((dm >> pd) & 1u))) {
+                double tau = st[0], T = st[NT], I = st[2 * NT];
+                rt_accumulate(dtau, em, phi, w, P.tau_max, tau, T, I);
+                st[0] = tau; st[NT] = T; st[2 * NT] = I; st[3 * NT] = a1; st[4 * NT] = e1;
+                // an accepted step that is not the ray's last one and leaves it opaque: the ray ends HERE (the
+                // geodesic may have run a few steps ahead; those are discarded)
+                int* const oq = sm_opq + (threadIdx.x & ~31) + o;
+                if ((meta & 0x300) == 0x200 && tau > P.tau_max && oq[0] < 0) { oq[0] = eatt; oq[NT] = eacc; }
+                mine = true;
+            }
+            __syncwarp();
+        }
+        f_head += (unsigned)nb;
+    };
+    // ---- a ray whose points have all been processed: outputs (kind 2, single frequency), the lane is free again
+    auto fifo_finalize = [&]() {
+        if (draining && (int)(f_head - my_last) > 0) {
+            int oflag = end_flag, oatt = n_att, oacc = n_acc;
+            if (sm_opq[threadIdx.x] >= 0) { oflag = F_OPAQUE; oatt = sm_opq[threadIdx.x]; oacc = sm_opq[NT + threadIdx.x]; }
+            if (O.flag) O.flag[pix] = oflag;
+            if (O.n_attempt) O.n_attempt[pix] = oatt;
+            if (O.n_accept) O.n_accept[pix] = oacc;
+            if (O.image) O.image[pix] = P.nu3[0] * RT1(2);
+            if (O.aux0) O.aux0[pix] = RT1(0);
+            if (O.aux1) O.aux1[pix] = 0.0;
+            draining = false;
+        }
+    };
 
     for (;;) {
         // ------------------------------------------------------------------ refill from the queue
-        const unsigned need = __ballot_sync(FULL, !active && !exhausted);
+        const bool want = !active && !exhausted && !(FIFO && draining);
+        const unsigned need = __ballot_sync(FULL, want);
         if (need) {
             const int leader = __ffs(need) - 1;
             unsigned long long base = 0;
             if (lane == leader) base = atomicAdd(O.queue, (unsigned long long)__popc(need));
             base = __shfl_sync(FULL, base, leader);
-            if (!active && !exhausted) {
+            if (want) {
                 const long long q = (long long)base + __popc(need & ((1u << lane) - 1u));
                 if (q >= P.n_queue) {
                     exhausted = true;
@@ -131,14 +224,23 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                                 RT1(0) = 0.0; RT1(1) = 1.0; RT1(2) = 0.0; RT1(3) = 0.0; RT1(4) = 0.0;
                             }
                         }
+                        if (FIFO) {
+                            sm_L[threadIdx.x] = L; sm_opq[threadIdx.x] = -1;
+                            my_last = f_head - 1u; prev_out = true;        // "previous point": already processed, outside the region
+                        }
                         active = true;
                     }
                 }
             }
         }
-        if (!__any_sync(FULL, active)) {
-            if (__all_sync(FULL, exhausted)) break;
-            continue;
+        const bool any_active = __any_sync(FULL, active);
+        if (!any_active) {
+            // (FIFO) no ray running but points waiting or lanes draining: fall through — the attempt below runs with every
+            // lane off (this happens only at the very end of the image), the ring is flushed, the drained lanes released
+            if (!(FIFO && (f_tail != f_head || __any_sync(FULL, draining)))) {
+                if (__all_sync(FULL, exhausted)) break;
+                continue;
+            }
         }
 
         // ------------------------------------------------------------------ one attempt
@@ -180,7 +282,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                 const double ts = stage_sum<TAB, I>(K, 4);                                                     \
                 rk_tau = fma(kRkB5[TAB][I], as, rk_tau);                                                       \
                 rk_I = fma(kRkB5[TAB][I] * es, d_exp_lo(-fma(h_try, ts, tau_n)), rk_I);                        \
-                K.set(4, I, as);                                                                               \
+                if (I < STAGE_SLOTS) K.set(4, I, as);                                                          \
             }                                                                                                  \
             store_stage<TAB, I>(K, k, ph5, phe);                                                               \
         }
@@ -189,7 +291,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         double yn_ph;
         {
             State yt, ye;
-            rk_combine<TAB>(K, y, h_try, ph5, phe, yt, ye);
+            rk_combine<TAB>(K, k, y, h_try, ph5, phe, yt, ye);
             const double err = error_norm(y, ye, P.inv_rtol);
             const bool normal = mode == M_NORMAL;
             const bool accepted = err <= 1.0;                          // a NaN is rejected
@@ -271,6 +373,31 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     nd[2] = make_double2(pt.u0, pt.ycoef); nd[3] = make_double2((double)n_att, 0.0);
                 }
             }
+        } else if (FIFO) {
+            // TRANSFER FIFO.  The coefficient evaluation at the end point of an accepted step is the most expensive
+            // part of a trip (~500 instructions) and only ~21 of the 32 lanes have such a point (rejected attempts,
+            // event-location retakes, rays outside the emitting region).  Nothing in the geodesic depends on it —
+            // only the OPAQUE ending does — so the points go into a per-warp ring in shared memory and are
+            // processed 32 at a time, one per lane, whichever lane they came from.  A ray that has ended waits
+            // (draining) until its last point has been processed before its pixel is written; a ray that turns out
+            // to be opaque has run ahead by the few steps still in the ring, which are discarded (its step counts
+            // are those recorded with the opaque step).
+            const bool step_pt = commit || fresh;
+            const bool inside = yn.r > P.r_cap && yn.r < P.r_rt_out;
+            // a point outside the emitting region whose predecessor was outside too contributes nothing
+            const bool push = step_pt && (inside || !prev_out || P.tau_max < 0.0);
+            const unsigned pm = __ballot_sync(FULL, push);
+            if (push) {
+                const unsigned pos = f_tail + __popc(pm & ((1u << lane) - 1u));
+                const int slot = (int)(pos & (FIFO_CAP - 1));
+                FD(0, slot) = yn.r; FD(1, slot) = sn; FD(2, slot) = cn; FD(3, slot) = yn.pr; FD(4, slot) = commit ? h_try : 0.0;
+                FI(0, slot) = lane | (flag >= 0 ? 0x100 : 0) | (commit ? 0x200 : 0);
+                FI(1, slot) = (int)my_last; FI(2, slot) = n_att; FI(3, slot) = n_acc;
+                my_last = pos; prev_out = !inside;
+            }
+            f_tail += __popc(pm);
+            __syncwarp();
+            if ((int)(f_tail - f_head) >= 32 || ((drain_wait >= 2 || !any_active) && f_tail != f_head)) { fifo_process(); drain_wait = 0; }
         } else if (KIND == 2 && (commit || fresh)) {
             RtPoint pt; rt_point<SPEC, PREC>(P, L, yn.r, sn, cn, yn.pr, pt);
             bool all_opaque = true;
@@ -317,7 +444,12 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         }
 
         // ------------------------------------------------------------------ ray ended: outputs, release the lane
-        if (flag >= 0) {
+        if (FIFO) {
+            if (active && flag < 0 && sm_opq[threadIdx.x] >= 0) flag = F_OPAQUE;        // found opaque by the ring: stop here
+            if (active && flag >= 0) { active = false; draining = true; end_flag = flag; }
+            fifo_finalize();
+            drain_wait = __any_sync(FULL, draining) ? drain_wait + 1 : 0;
+        } else if (flag >= 0) {
             if (O.flag) O.flag[pix] = flag;
             if (O.r) O.r[pix] = y.r;
             if (O.th) O.th[pix] = y.th;
@@ -404,6 +536,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     }
 #undef ACC
 #undef RT1
+#undef FD
+#undef FI
     // ---------------------------------------------------------------------- block-level reductions
     if ((SPEC || KIND == 4) && O.nuLnu) {
         __syncthreads();
