@@ -91,6 +91,7 @@ int check_scene(const odyssey_scene* S) {
         return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown tableau %d", S->tableau);
     if (!(S->r_obs > 0.0) || !(S->h0 > 0.0) || !(S->r_esc > 0.0) || !(S->horizon_eps >= 0.0) || S->max_attempts <= 0)
         return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "r_obs, h0, r_esc, max_attempts must be positive and horizon_eps >= 0");
+    if (S->max_attempts >= (1 << FIFO_ACC_BITS)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "max_attempts = %d must be below 2^%d", S->max_attempts, FIFO_ACC_BITS);
     if (!(S->x_max > S->x_min) || !(S->y_max > S->y_min))
         return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "image-plane extent is empty");
     {   // every ray must come back out through r = r_esc: a ray whose impact parameter exceeds r_esc turns around
@@ -216,7 +217,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
 
 // ---- kernel table ------------------------------------------------------------------------------
 #ifndef ODY_MINB_MAIN
-#define ODY_MINB_MAIN 5
+#define ODY_MINB_MAIN 5                         // (-DODY_MINB_MAIN=4 builds the 128-register variant of the occupancy comparison in DESIGN.md)
 #endif
 constexpr int NT_MAIN = 128, MINB_MAIN = ODY_MINB_MAIN;     // 96 registers per thread at most
 constexpr int MINB_SPOT = 4;                    // hot spot (kind 3, with the coordinate time) and Novikov-Thorne disk (kind 4): 4 blocks per SM keep them free of spills

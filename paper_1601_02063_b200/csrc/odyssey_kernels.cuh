@@ -59,16 +59,18 @@ __device__ __forceinline__ void store_stage(KS& K, const Slope& k, double& ph5, 
 __host__ __device__ constexpr int smem_per_thread(int rts) { return (rts == 1 ? STAGE_ROWS : STAGE_ROWS - 1) * STAGE_SLOTS + 5; }
 
 // Transfer FIFO (single-frequency per-step scheme): per warp a ring of FIFO_CAP points waiting for their
-// absorption / emission coefficients — 5 doubles (r, sinθ, cosθ, p_r, step length) and 4 ints (owner lane | flags,
-// position of the owner's previous point, attempted and accepted step counts) each — plus, per thread, the ray's L
-// and the step counts at which the ray turned opaque.
+// absorption / emission coefficients — 5 doubles (r, sinθ, cosθ, p_r, step length) and 2 ints (attempted step count;
+// accepted step count | owner lane << 25 | "last step of the ray" << 30 | "accepted step" << 31) each — plus, per
+// thread, the ray's L and four ints: the step counts at which the ray turned opaque, the ring position of the
+// lane's latest point, the outcome of a ray that has ended.
 #ifndef ODY_RT_FIFO
 #define ODY_RT_FIFO 1
 #endif
 constexpr int FIFO_CAP = 64;
 constexpr int FIFO_DOUBLES = 7 * FIFO_CAP;                               // per warp
+constexpr int FIFO_ACC_BITS = 25;                                        // accepted-step counts below 2^25 (check_scene)
 __host__ __device__ constexpr bool uses_fifo(int kind, bool spec, int rts) { return ODY_RT_FIFO && kind == 2 && !spec && rts == 0; }
-__host__ __device__ constexpr int fifo_doubles_per_block(int nt) { return nt + (nt / 32) * FIFO_DOUBLES + nt; }   // L, rings, 2 ints per thread
+__host__ __device__ constexpr int fifo_doubles_per_block(int nt) { return nt + (nt / 32) * FIFO_DOUBLES + 2 * nt; }
 
 // RTS = 1: transfer scheme E' (tau, I as Runge–Kutta components; single frequency only).
 // RTS = 2: record mode, the first phase of the two-phase spectrum path (see spectrum_rt_kernel below).
@@ -101,13 +103,14 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     constexpr bool FIFO = uses_fifo(KIND, SPEC, RTS);
     double* const sm_L = sm_red;                                                          // [NT] L of the lane's ray
     double* const sm_ring = sm_red + NT + (threadIdx.x >> 5) * FIFO_DOUBLES;              // this warp's ring
-    int* const sm_ringi = reinterpret_cast<int*>(sm_ring + 5 * FIFO_CAP);
-    int* const sm_opq = reinterpret_cast<int*>(sm_red + NT + (NT / 32) * FIFO_DOUBLES);   // [2][NT]: n_attempt, n_accept at the opaque crossing
+    int4* const sm_ringi = reinterpret_cast<int4*>(sm_ring + 5 * FIFO_CAP);
+    int* const sm_lane = reinterpret_cast<int*>(sm_red + NT + (NT / 32) * FIFO_DOUBLES);  // [4][NT] ints, see the Q_ indices
+    constexpr int Q_OATT = 0, Q_OACC = 1, Q_LAST = 2, Q_END = 3;                          // opaque crossing: n_attempt (-1: none), n_accept; latest ring position; end flag
     double* const sm_rtw = smem + (smem_per_thread(RTS) - 5) * NT + (threadIdx.x & ~31);  // RT state of this warp's lane 0
 #define FD(f, slot) sm_ring[(f) * FIFO_CAP + (slot)]
-#define FI(g, slot) sm_ringi[(g) * FIFO_CAP + (slot)]
-    unsigned f_head = 0, f_tail = 0, my_last = 0u - 1u;                                   // ring positions (warp-uniform head, tail)
-    int drain_wait = 0, end_flag = -1;
+#define LN(q) sm_lane[(q) * NT + threadIdx.x]
+    unsigned f_head = 0, f_tail = 0;                                                      // ring positions (warp-uniform)
+    int drain_wait = 0;
     bool draining = false, prev_out = true;
 
     const double a = P.a, a2 = P.a2;
@@ -136,12 +139,9 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         const bool have = lane < nb;
         const int slot = (int)((f_head + lane) & (FIFO_CAP - 1));
         double er = 0.0, esn = 0.0, ecn = 0.0, epr = 0.0, eh = 0.0;
-        int meta = 0, prevpos = 0, eatt = 0, eacc = 0;
-        if (have) {
-            er = FD(0, slot); esn = FD(1, slot); ecn = FD(2, slot); epr = FD(3, slot); eh = FD(4, slot);
-            meta = FI(0, slot); prevpos = FI(1, slot); eatt = FI(2, slot); eacc = FI(3, slot);
-        }
-        const int o = meta & 31;
+        int4 meta = make_int4(0, 0, 0, 0);
+        if (have) { er = FD(0, slot); esn = FD(1, slot); ecn = FD(2, slot); epr = FD(3, slot); eh = FD(4, slot); meta = sm_ringi[slot]; }
+        const int o = (meta.y >> FIFO_ACC_BITS) & 31;
         double a1 = 0.0, e1 = 0.0;
         if (have) {
             RtPoint pt; rt_point<false, PREC>(P, sm_L[(threadIdx.x & ~31) + o], er, esn, ecn, epr, pt);
@@ -149,12 +149,12 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             FD(0, slot) = a1; FD(1, slot) = e1;
         }
         __syncwarp();
-        const int pd = (int)((unsigned)prevpos - f_head);            // >= 0: the owner's previous point is in this batch
+        const int pd = (int)((unsigned)meta.z - f_head);             // >= 0: the owner's previous point is in this batch, pd lanes up
         double* const st = sm_rtw + o;                                // the owner's tau, T, I, a0, e0
         double dtau = 0.0, em = 0.0, phi = 1.0, w = 0.0;
         if (have) {
             double a0, e0;
-            if (pd >= 0) { const int ps = prevpos & (FIFO_CAP - 1); a0 = FD(0, ps); e0 = FD(1, ps); }
+            if (pd >= 0) { const int ps = (int)((f_head + pd) & (FIFO_CAP - 1)); a0 = FD(0, ps); e0 = FD(1, ps); }
             else { a0 = st[3 * NT]; e0 = st[4 * NT]; }
             rt_increments<PREC>(a0, a1, e0, e1, eh, dtau, em, phi, w);
         }
@@ -165,11 +165,14 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             if (!mine && (pd < 0 || ((dm >> pd) & 1u))) {
                 double tau = st[0], T = st[NT], I = st[2 * NT];
                 rt_accumulate(dtau, em, phi, w, P.tau_max, tau, T, I);
-                st[0] = tau; st[NT] = T; st[2 * NT] = I; st[3 * NT] = a1; st[4 * NT] = e1;
+                st[0] = tau; st[NT] = T; st[2 * NT] = I;
+                st[3 * NT] = a1; st[4 * NT] = e1;
                 // an accepted step that is not the ray's last one and leaves it opaque: the ray ends HERE (the
                 // geodesic may have run a few steps ahead; those are discarded)
-                int* const oq = sm_opq + (threadIdx.x & ~31) + o;
-                if ((meta & 0x300) == 0x200 && tau > P.tau_max && oq[0] < 0) { oq[0] = eatt; oq[NT] = eacc; }
+                if (meta.y < 0 && !(meta.y & (1 << 30)) && tau > P.tau_max) {
+                    int* const oq = sm_lane + (threadIdx.x & ~31) + o;
+                    if (oq[Q_OATT * NT] < 0) { oq[Q_OATT * NT] = meta.x; oq[Q_OACC * NT] = meta.y & ((1 << FIFO_ACC_BITS) - 1); }
+                }
                 mine = true;
             }
             __syncwarp();
@@ -178,9 +181,9 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     };
     // ---- a ray whose points have all been processed: outputs (kind 2, single frequency), the lane is free again
     auto fifo_finalize = [&]() {
-        if (draining && (int)(f_head - my_last) > 0) {
-            int oflag = end_flag, oatt = n_att, oacc = n_acc;
-            if (sm_opq[threadIdx.x] >= 0) { oflag = F_OPAQUE; oatt = sm_opq[threadIdx.x]; oacc = sm_opq[NT + threadIdx.x]; }
+        if (draining && (int)(f_head - (unsigned)LN(Q_LAST)) > 0) {
+            int oflag = LN(Q_END), oatt = n_att, oacc = n_acc;
+            if (LN(Q_OATT) >= 0) { oflag = F_OPAQUE; oatt = LN(Q_OATT); oacc = LN(Q_OACC); }
             if (O.flag) O.flag[pix] = oflag;
             if (O.n_attempt) O.n_attempt[pix] = oatt;
             if (O.n_accept) O.n_accept[pix] = oacc;
@@ -225,8 +228,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                             }
                         }
                         if (FIFO) {
-                            sm_L[threadIdx.x] = L; sm_opq[threadIdx.x] = -1;
-                            my_last = f_head - 1u; prev_out = true;        // "previous point": already processed, outside the region
+                            sm_L[threadIdx.x] = L; LN(Q_OATT) = -1;
+                            LN(Q_LAST) = (int)(f_head - 1u); prev_out = true;   // "latest point": already processed, outside the region
                         }
                         active = true;
                     }
@@ -391,9 +394,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                 const unsigned pos = f_tail + __popc(pm & ((1u << lane) - 1u));
                 const int slot = (int)(pos & (FIFO_CAP - 1));
                 FD(0, slot) = yn.r; FD(1, slot) = sn; FD(2, slot) = cn; FD(3, slot) = yn.pr; FD(4, slot) = commit ? h_try : 0.0;
-                FI(0, slot) = lane | (flag >= 0 ? 0x100 : 0) | (commit ? 0x200 : 0);
-                FI(1, slot) = (int)my_last; FI(2, slot) = n_att; FI(3, slot) = n_acc;
-                my_last = pos; prev_out = !inside;
+                sm_ringi[slot] = make_int4(n_att, n_acc | (lane << FIFO_ACC_BITS) | (flag >= 0 ? 1 << 30 : 0) | (commit ? 1 << 31 : 0), LN(Q_LAST), 0);
+                LN(Q_LAST) = (int)pos; prev_out = !inside;
             }
             f_tail += __popc(pm);
             __syncwarp();
@@ -445,8 +447,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
 
         // ------------------------------------------------------------------ ray ended: outputs, release the lane
         if (FIFO) {
-            if (active && flag < 0 && sm_opq[threadIdx.x] >= 0) flag = F_OPAQUE;        // found opaque by the ring: stop here
-            if (active && flag >= 0) { active = false; draining = true; end_flag = flag; }
+            if (active && flag < 0 && LN(Q_OATT) >= 0) flag = F_OPAQUE;                 // found opaque by the ring: stop here
+            if (active && flag >= 0) { active = false; draining = true; LN(Q_END) = flag; }
             fifo_finalize();
             drain_wait = __any_sync(FULL, draining) ? drain_wait + 1 : 0;
         } else if (flag >= 0) {
@@ -537,7 +539,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
 #undef ACC
 #undef RT1
 #undef FD
-#undef FI
+#undef LN
     // ---------------------------------------------------------------------- block-level reductions
     if ((SPEC || KIND == 4) && O.nuLnu) {
         __syncthreads();
