@@ -25,15 +25,16 @@
  *   - Return value: ODYSSEY_OK (0) or a negative odyssey_status.  After a failure
  *     odyssey_last_error() returns a static, thread-local, NUL-terminated description.
  *     Nothing is printed, nothing throws.
- *   - The library owns a small ring of 64 work-queue counters per device (allocated lazily, released
- *     by odyssey_shutdown(); every launch takes the next one, so up to 64 launches may be in flight at
- *     once) and takes its scratch (initial states: 48 bytes per pixel; spectrum mode: see there) from
- *     the device's default stream-ordered memory pool (cudaMallocAsync / cudaFreeAsync on `cuda_stream`).
- *   - Every call first runs a camera kernel (initial conditions of all pixels), then the persistent
- *     integrator kernel: two kernel launches of this library per call (more in spectrum mode).
- *   - All of that is stream-ordered, so a DEVICE call may be captured into a CUDA graph and replayed (the captured
- *     graph keeps the call's queue counter: replay it on one stream at a time).  The exception is the two-phase path
- *     of odyssey_render_spectrum, which synchronises the stream inside the call.
+ *   - Scratch: every launch takes what it needs — its work-queue counter, one stash of 32 prepared rays per
+ *     warp of the grid (~5 MB in all, whatever the image size), in spectrum mode the per-frequency accumulators
+ *     or node lists described there — from a stream-ordered memory pool of the library's own (created lazily per
+ *     device, cudaMallocFromPoolAsync / cudaFreeAsync on `cuda_stream`; cached blocks above 6 GiB go back to the
+ *     driver at the next synchronisation; odyssey_trim_scratch() returns more, odyssey_shutdown() everything).
+ *     Nothing is shared between launches, so any number of calls may be in flight on any number of streams.
+ *   - One kernel launch of this library per call (the persistent integrator builds the initial conditions of its
+ *     rays itself, a queue tile of 32 pixels at a time); more in spectrum mode.
+ *   - All of that is stream-ordered, so a DEVICE call may be captured into a CUDA graph and replayed.  The exception
+ *     is the two-phase path of odyssey_render_spectrum, which synchronises the stream inside the call.
  */
 #ifndef ODYSSEY_H_
 #define ODYSSEY_H_
@@ -70,8 +71,8 @@ enum { ODYSSEY_KIND_NONE = 0, ODYSSEY_KIND_THIN_DISK = 1, ODYSSEY_KIND_RIAF = 2,
 enum { ODYSSEY_RT_PER_STEP = 0, ODYSSEY_RT_RK_COMPONENTS = 1 };
 /* FP64: everything in double precision (default).  MIXED_FP32: the geodesic, every exponent sum, argument
  * reduction and accumulator stay FP64; the polynomial cores of exp / expm1 / log and the K_2 polynomials of the
- * emissivity run in FP32 (relative error ~1e-7 per coefficient).  Offered for measurement: on B200 it is not
- * faster.                                                                            */
+ * emissivity run in FP32 (relative error ~1e-7 per coefficient).  Inside the image tolerances and a few per cent
+ * faster on B200; not the default: the metric is FP64.                                 */
 enum { ODYSSEY_PREC_FP64 = 0, ODYSSEY_PREC_MIXED_FP32 = 1 };
 #define ODYSSEY_MAX_FREQ 32
 
@@ -207,6 +208,10 @@ int odyssey_eval_math(int op, int n, const double* x, double* y, double* y2, voi
 
 /* Number of kernel launches issued by this library since load (for bench.py's gpu_launches). */
 long long odyssey_launch_count(void);
+
+/* Synchronises the current device and returns the library's cached scratch above keep_bytes to the driver
+ * (e.g. 0 after a large two-phase spectrum call, before another library needs the memory). */
+int odyssey_trim_scratch(unsigned long long keep_bytes);
 
 const char* odyssey_last_error(void);
 void odyssey_shutdown(void);

@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = (
     "odyssey_trace_geodesics", "odyssey_render_image", "odyssey_render_spectrum", "odyssey_render_hotspot",
     "odyssey_trace_geodesics_host", "odyssey_render_image_host", "odyssey_render_spectrum_host",
     "odyssey_render_hotspot_host",
-    "odyssey_fp64_peak_probe", "odyssey_kernel_info", "odyssey_eval_math", "odyssey_launch_count",
+    "odyssey_fp64_peak_probe", "odyssey_kernel_info", "odyssey_eval_math", "odyssey_trim_scratch", "odyssey_launch_count",
     "odyssey_last_error", "odyssey_shutdown",
 )
 
@@ -95,7 +95,8 @@ def load_library():
                                          dp, dp, dp, dp, dp, dp, dp, ip, ip, vp]
     L.odyssey_render_hotspot_host.argtypes = [C.POINTER(Scene), C.POINTER(Model), C.POINTER(C.c_double), C.c_int,
                                               dp, dp, dp, dp, dp, dp, dp, ip, ip]
-    for name in EXPORTED_SYMBOLS[:11]:
+    L.odyssey_trim_scratch.argtypes = [C.c_ulonglong]
+    for name in EXPORTED_SYMBOLS[:12]:
         getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -292,6 +293,11 @@ def kernel_info(kind, spectrum=False, tableau=0):
                                               *[C.byref(x) for x in v]))
     return dict(registers=v[0].value, local_bytes=v[1].value, threads_per_block=v[2].value,
                 blocks_per_sm=v[3].value, n_sm=v[4].value)
+
+
+def trim_scratch(keep_bytes=0):
+    """odyssey_trim_scratch: give the library's cached device scratch above keep_bytes back to the driver."""
+    _check(load_library().odyssey_trim_scratch(C.c_ulonglong(int(keep_bytes))))
 
 
 def launch_count():

@@ -37,9 +37,11 @@ int fail(int code, const char* fmt, ...) {
     do { cudaError_t e_ = (expr);                                                                  \
          if (e_ != cudaSuccess) return fail(ODYSSEY_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } while (0)
 
-// ---- per-device library state: SM count and a ring of queue counters --------------------------
-constexpr int MAX_DEV = 16, RING = 64;
-struct DevState { bool ready = false; int n_sm = 0; unsigned long long* ring = nullptr; unsigned next = 0; };
+// ---- per-device library state: SM count ---------------------------------------------------------
+// (Every launch takes its work-queue counter and the warps' ray stashes from stream-ordered scratch of its own, so
+// any number of calls may be in flight on any number of streams, and a captured graph owns what it captured.)
+constexpr int MAX_DEV = 16;
+struct DevState { bool ready = false; int n_sm = 0; cudaMemPool_t pool = nullptr; };
 DevState g_dev[MAX_DEV];
 std::mutex g_mu;
 
@@ -55,23 +57,35 @@ int device_state(DevState** out, int* dev_out) {
         if (prop.major != 10)
             return fail(ODYSSEY_ERR_UNSUPPORTED_DEVICE, "device %d is sm_%d%d; this library is built for sm_100a only", dev, prop.major, prop.minor);
         D.n_sm = prop.multiProcessorCount;
-        CUDA_TRY(cudaMalloc(&D.ring, RING * sizeof(unsigned long long)));
-        // stream-ordered scratch (spectrum accumulators, the _host variants' device buffers) comes from the
-        // device's default pool; keep freed blocks cached instead of returning them at every synchronisation
-        cudaMemPool_t pool = nullptr;
-        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-            unsigned long long keep = ~0ull;
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        }
+        // Stream-ordered scratch (queue counters, ray stashes, spectrum accumulators and node lists, the _host variants'
+        // device buffers) comes from a memory pool of the library's OWN, which keeps freed blocks cached instead of
+        // returning them to the driver at every synchronisation; the device's default pool, which belongs to the host
+        // application, is not touched.
+        cudaMemPoolProps props;
+        std::memset(&props, 0, sizeof(props));
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        CUDA_TRY(cudaMemPoolCreate(&D.pool, &props));
+        unsigned long long keep = 6ull << 30;      // cached scratch above 6 GiB goes back to the driver at the next synchronisation
+        CUDA_TRY(cudaMemPoolSetAttribute(D.pool, cudaMemPoolAttrReleaseThreshold, &keep));
         D.ready = true;
     }
     *out = &D; if (dev_out) *dev_out = dev;
     return ODYSSEY_OK;
 }
 
-unsigned long long* next_counter(DevState* D) {
-    std::lock_guard<std::mutex> lk(g_mu);
-    return D->ring + (D->next++ % RING);
+// stream-ordered allocation from the library's pool on the current device
+cudaError_t pool_alloc(void** ptr, size_t bytes, cudaStream_t st) {
+    DevState* D = nullptr;
+    if (device_state(&D, nullptr) != ODYSSEY_OK) return cudaErrorInitializationError;
+    return cudaMallocFromPoolAsync(ptr, bytes, D->pool, st);
+}
+// give cached blocks above `keep_bytes` back to the driver (after the calls that take gigabytes of scratch)
+void pool_trim(size_t keep_bytes) {
+    DevState* D = nullptr;
+    if (device_state(&D, nullptr) == ODYSSEY_OK && D->pool) cudaMemPoolTrimTo(D->pool, keep_bytes);
 }
 
 // ---- Kerr constants (Bardeen, Press & Teukolsky 1972, cited PAPER.md:L223) -----------------------
@@ -275,34 +289,21 @@ int launch(const Params& P, Outputs O, bool spec, int tab, cudaStream_t st) {
     const long long blocks_needed = (warps_needed + nt / 32 - 1) / (nt / 32);
     if (blocks > blocks_needed) blocks = blocks_needed;
     if (blocks < 1) blocks = 1;
-    O.queue = next_counter(D);
-    CUDA_TRY(cudaMemsetAsync(O.queue, 0, sizeof(unsigned long long), st));
     if (O.hist && P.nbins > 0) CUDA_TRY(cudaMemsetAsync(O.hist, 0, sizeof(double) * P.nbins, st));
     if (O.nuLnu) CUDA_TRY(cudaMemsetAsync(O.nuLnu, 0, sizeof(double) * P.nf, st));
-    // camera pass: initial state of every queue slot, at full lane efficiency, into stream-ordered scratch
-    double* init_state = nullptr;
-    if (!O.init_state) {
-        CUDA_TRY(cudaMallocAsync((void**)&init_state, sizeof(double) * 6 * (size_t)P.n_queue, st));
-        const long long ib = std::min<long long>((P.n_queue + 255) / 256, (long long)D->n_sm * 16);
-        init_rays_kernel<<<(unsigned)ib, 256, 0, st>>>(P, init_state);
-        cudaError_t ie = cudaGetLastError();
-        if (ie != cudaSuccess) { cudaFreeAsync(init_state, st); return fail(ODYSSEY_ERR_CUDA, "init_rays_kernel: %s", cudaGetErrorString(ie)); }
-        g_launches.fetch_add(1);
-        O.init_state = init_state;
-    }
-    if (spec) {      // stream-ordered scratch for the per-frequency accumulators: [5][nf][blocks * nt] doubles
-        void* scratch = nullptr;
-        cudaError_t se = cudaMallocAsync(&scratch, sizeof(double) * 5 * (size_t)P.nf * (size_t)blocks * nt, st);
-        if (se != cudaSuccess) {
-            if (init_state) cudaFreeAsync(init_state, st);
-            return fail(ODYSSEY_ERR_CUDA, "spectrum scratch: %s", cudaGetErrorString(se));
-        }
-        O.spec_state = (double*)scratch;
-    }
+    // stream-ordered scratch of this launch: the work-queue counter (its own 256 bytes), one stash of 32 prepared
+    // rays per warp of the grid and, in spectrum mode, the per-frequency accumulators [5][nf][blocks * nt]
+    const size_t stash_bytes = (size_t)blocks * (nt / 32) * STASH_DOUBLES * sizeof(double);
+    const size_t spec_bytes = spec ? sizeof(double) * 5 * (size_t)P.nf * (size_t)blocks * nt : 0;
+    char* scratch = nullptr;
+    CUDA_TRY(pool_alloc((void**)&scratch, 256 + stash_bytes + spec_bytes, st));
+    O.queue = reinterpret_cast<unsigned long long*>(scratch);
+    O.stash = reinterpret_cast<double*>(scratch + 256);
+    if (spec) O.spec_state = reinterpret_cast<double*>(scratch + 256 + stash_bytes);
+    cudaError_t le = cudaMemsetAsync(O.queue, 0, sizeof(unsigned long long), st);
     void* args[] = {(void*)&P, (void*)&O};
-    cudaError_t le = cudaLaunchKernel((const void*)fn, dim3((unsigned)blocks), dim3(nt), args, sm, st);
-    if (spec) cudaFreeAsync(O.spec_state, st);
-    if (init_state) cudaFreeAsync(init_state, st);
+    if (le == cudaSuccess) le = cudaLaunchKernel((const void*)fn, dim3((unsigned)blocks), dim3(nt), args, sm, st);
+    cudaFreeAsync(scratch, st);
     if (le != cudaSuccess) return fail(ODYSSEY_ERR_CUDA, "cudaLaunchKernel: %s", cudaGetErrorString(le));
     g_launches.fetch_add(1);
     return ODYSSEY_OK;
@@ -333,25 +334,27 @@ int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st, 
     TRY_RC(device_state(&D, nullptr));
     const size_t n = (size_t)P.nx * P.ny;
     int32_t *iflag = nullptr, *iatt = nullptr, *iacc = nullptr; long long* off = nullptr; double* nodes = nullptr;
+    unsigned long long* counter2 = nullptr;                                       // the transfer kernel's own ray counter
     auto release = [&]() {
+        if (counter2) cudaFreeAsync(counter2, st);
         if (iflag) cudaFreeAsync(iflag, st); if (iatt) cudaFreeAsync(iatt, st); if (iacc) cudaFreeAsync(iacc, st);
         if (off) cudaFreeAsync(off, st); if (nodes) cudaFreeAsync(nodes, st);
     };
 #define TP_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { release(); return fail(ODYSSEY_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_)); } } while (0)
-    TP_TRY(cudaMallocAsync((void**)&iflag, n * sizeof(int32_t), st));
-    TP_TRY(cudaMallocAsync((void**)&iatt, n * sizeof(int32_t), st));
-    TP_TRY(cudaMallocAsync((void**)&iacc, n * sizeof(int32_t), st));
-    TP_TRY(cudaMallocAsync((void**)&off, (n + 1) * sizeof(long long), st));
+    TP_TRY(pool_alloc((void**)&iflag, n * sizeof(int32_t), st));
+    TP_TRY(pool_alloc((void**)&iatt, n * sizeof(int32_t), st));
+    TP_TRY(pool_alloc((void**)&iacc, n * sizeof(int32_t), st));
+    TP_TRY(pool_alloc((void**)&off, (n + 1) * sizeof(long long), st));
     Params Pr = P; Pr.rt_scheme = 2; Pr.nf = 1;
     Outputs O1 = no_outputs();
     O1.flag = iflag; O1.n_attempt = iatt; O1.n_accept = iacc;
     // First try: ONE record pass into fixed-capacity node lists (NODE_CAP nodes per ray) and an overflow flag.
     int32_t* ovf = nullptr;
-    TP_TRY(cudaMallocAsync((void**)&ovf, sizeof(int32_t), st));
+    TP_TRY(pool_alloc((void**)&ovf, sizeof(int32_t), st));
     TP_TRY(cudaMemsetAsync(ovf, 0, sizeof(int32_t), st));
     int rc = ODYSSEY_OK;
     int32_t overflow = 0;
-    if (cudaMallocAsync((void**)&nodes, n * NODE_CAP * NODE_DOUBLES * sizeof(double), st) != cudaSuccess) {
+    if (pool_alloc((void**)&nodes, n * NODE_CAP * NODE_DOUBLES * sizeof(double), st) != cudaSuccess) {
         cudaGetLastError();                                                    // no room for fixed-capacity lists:
         nodes = nullptr; overflow = 1;                                         // size them exactly instead
     } else {
@@ -380,7 +383,7 @@ int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st, 
         long long total = 0;
         TP_TRY(cudaMemcpyAsync(&total, off + n, sizeof(long long), cudaMemcpyDeviceToHost, st));
         TP_TRY(cudaStreamSynchronize(st));
-        TP_TRY(cudaMallocAsync((void**)&nodes, (size_t)total * NODE_DOUBLES * sizeof(double), st));
+        TP_TRY(pool_alloc((void**)&nodes, (size_t)total * NODE_DOUBLES * sizeof(double), st));
         O1.nodes = nodes; O1.node_offset = off;
         rc = launch(Pr, O1, false, tab, st);
         if (rc) { release(); return rc; }
@@ -389,7 +392,8 @@ int render_spectrum_two_phase(Params P, Outputs user, int tab, cudaStream_t st, 
     Outputs O2 = no_outputs();
     O2.images = user.images; O2.nuLnu = user.nuLnu; O2.flag = user.flag; O2.n_attempt = user.n_attempt;
     O2.nodes = nodes; O2.node_offset = off; O2.node_cap = node_cap; O2.aux_nacc = iacc; O2.image_stride = user.image_stride;
-    O2.queue = next_counter(D);
+    TP_TRY(pool_alloc((void**)&counter2, 256, st));
+    O2.queue = counter2;
     TP_TRY(cudaMemsetAsync(O2.queue, 0, sizeof(unsigned long long), st));
     if (user.nuLnu && zero_sed) TP_TRY(cudaMemsetAsync(user.nuLnu, 0, sizeof(double) * P.nf, st));
     if (user.flag) TP_TRY(cudaMemcpyAsync(user.flag, iflag, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
@@ -426,7 +430,7 @@ struct Scratch {
         *out = nullptr;
         if (!host_ptr) return ODYSSEY_OK;
         void* d = nullptr;
-        CUDA_TRY(cudaMallocAsync(&d, count * sizeof(T), 0));
+        CUDA_TRY(pool_alloc(&d, count * sizeof(T), 0));
         dev[n] = d; host[n] = host_ptr; bytes[n] = count * sizeof(T); ++n;
         *out = (T*)d;
         return ODYSSEY_OK;
@@ -655,6 +659,14 @@ int odyssey_kernel_info(int kind, int spectrum, int tableau, int32_t* regs, int3
 
 long long odyssey_launch_count(void) { return g_launches.load(); }
 
+int odyssey_trim_scratch(unsigned long long keep_bytes) {
+    DevState* D = nullptr;
+    TRY(device_state(&D, nullptr));
+    CUDA_TRY(cudaDeviceSynchronize());
+    pool_trim((size_t)keep_bytes);
+    return ODYSSEY_OK;
+}
+
 const char* odyssey_last_error(void) { return g_err; }
 
 void odyssey_shutdown(void) {
@@ -664,9 +676,8 @@ void odyssey_shutdown(void) {
     for (int d = 0; d < MAX_DEV; ++d) {
         if (!g_dev[d].ready) continue;
         cudaSetDevice(d);
-        cudaFree(g_dev[d].ring);
-        cudaMemPool_t pool = nullptr;
-        if (cudaDeviceGetDefaultMemPool(&pool, d) == cudaSuccess) { cudaDeviceSynchronize(); cudaMemPoolTrimTo(pool, 0); }
+        cudaDeviceSynchronize();
+        if (g_dev[d].pool) cudaMemPoolDestroy(g_dev[d].pool);
         g_dev[d] = DevState();
     }
     cudaSetDevice(cur);

@@ -113,6 +113,11 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     int drain_wait = 0;
     bool draining = false, prev_out = true;
 
+    // the warp's stash of prepared rays (see the refill): [7][32] doubles of scratch
+    double* const stash = O.stash + ((size_t)blockIdx.x * (NT / 32) + (threadIdx.x >> 5)) * STASH_DOUBLES;
+    int st_cnt = 0;                                                                       // prepared rays left (warp-uniform)
+    bool queue_done = false;                                                              // the queue has handed out its last tile
+
     const double a = P.a, a2 = P.a2;
     bool active = false, exhausted = false, on_eq = false;
     int pix = 0, n_att = 0, n_acc = 0, mode = M_NORMAL, loc_it = 0;
@@ -196,45 +201,65 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
 
     for (;;) {
         // ------------------------------------------------------------------ refill from the queue
+        // A lane whose ray has ended takes its next one from the warp's STASH of prepared rays.  The initial
+        // conditions (§2.2: ~700 instructions with acos, atan2, two sincos and the square roots) are not
+        // built lane by lane as rays end — that would run ~1.5 lanes wide — but 32 at a time: when the stash is
+        // empty the warp takes one whole queue tile (8 x 4 pixels) with ONE atomicAdd and every lane, busy or
+        // not, builds the state of one of its pixels.  The stash is 32 x 7 doubles per warp of stream-ordered
+        // scratch (a few MB for the whole grid: it lives in L2), so there is no camera kernel, no per-pixel
+        // scratch and no HBM traffic beyond the outputs.
         const bool want = !active && !exhausted && !(FIFO && draining);
         const unsigned need = __ballot_sync(FULL, want);
         if (need) {
-            const int leader = __ffs(need) - 1;
-            unsigned long long base = 0;
-            if (lane == leader) base = atomicAdd(O.queue, (unsigned long long)__popc(need));
-            base = __shfl_sync(FULL, base, leader);
-            if (want) {
-                const long long q = (long long)base + __popc(need & ((1u << lane) - 1u));
-                if (q >= P.n_queue) {
-                    exhausted = true;
-                } else {
-                    const int tile = (int)(q >> 5), w = (int)(q & 31);
-                    const int i = (tile % P.tiles_x) * TILE_W + (w & (TILE_W - 1));
-                    const int j = (tile / P.tiles_x) * TILE_H + (w / TILE_W);
-                    if (i < P.nx && j < P.ny) {
-                        // initial state and L of queue slot q, built at full lane efficiency by init_rays_kernel
-                        // ([6][n_queue] doubles; a refill here runs ~1.5 lanes wide, so no arithmetic is done here)
-                        const double* st = O.init_state + q;
-                        y.r = __ldg(st); y.th = __ldg(st + P.n_queue); y.ph = __ldg(st + 2 * P.n_queue);
-                        y.pr = __ldg(st + 3 * P.n_queue); y.pth = __ldg(st + 4 * P.n_queue); L = __ldg(st + 5 * P.n_queue);
-                        pix = j * P.nx + i;
-                        n_att = 0; n_acc = 0; mode = M_FRESH; loc_it = 0; on_eq = false; y_t = 0.0;
-                        h_try = P.h0; h_next = P.h0; g_disk = 0.0; r_e = 0.0;
-                        if (KIND == 2) {
-                            if (SPEC) {
-                                for (int k = 0; k < nf; ++k) { ACC(0, k) = 0.0; ACC(1, k) = 1.0; ACC(2, k) = 0.0; ACC(3, k) = 0.0; ACC(4, k) = 0.0; }
-                            } else {
-                                RT1(0) = 0.0; RT1(1) = 1.0; RT1(2) = 0.0; RT1(3) = 0.0; RT1(4) = 0.0;
-                            }
-                        }
-                        if (FIFO) {
-                            sm_L[threadIdx.x] = L; LN(Q_OATT) = -1;
-                            LN(Q_LAST) = (int)(f_head - 1u); prev_out = true;   // "latest point": already processed, outside the region
-                        }
-                        active = true;
+            if (st_cnt == 0 && !queue_done) {
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(O.queue, 32ull);
+                base = __shfl_sync(FULL, base, 0);
+                queue_done = (long long)base + 32 >= P.n_queue;
+                const long long q = (long long)base + lane;
+                const int tile = (int)(q >> 5), w = (int)(q & 31);
+                const int i = (tile % P.tiles_x) * TILE_W + (w & (TILE_W - 1));
+                const int j = (tile / P.tiles_x) * TILE_H + (w / TILE_W);
+                const bool valid = q < P.n_queue && i < P.nx && j < P.ny;        // (a ragged image edge leaves tile slots empty)
+                const unsigned vm = __ballot_sync(FULL, valid);
+                if (valid) {
+                    const double x = P.x_min + (i + 0.5) * P.x_span / P.nx;      // pixel centres (reading K)
+                    const double yy = P.y_min + (j + P.row0 + 0.5) * P.y_span / P.ny_image;
+                    State y0; double L0;
+                    init_ray(P, x, yy, y0, L0);
+                    const int idx = __popc(vm & ((1u << lane) - 1u));
+                    stash[idx] = y0.r; stash[32 + idx] = y0.th; stash[64 + idx] = y0.ph; stash[96 + idx] = y0.pr;
+                    stash[128 + idx] = y0.pth; stash[160 + idx] = L0; stash[192 + idx] = __longlong_as_double((long long)(j * P.nx + i));
+                }
+                st_cnt = __popc(vm);
+                __syncwarp();
+            }
+            const int rank = __popc(need & ((1u << lane) - 1u));
+            if (want && rank < st_cnt) {
+                const double* st = stash + (st_cnt - 1 - rank);
+                y.r = __ldcg(st); y.th = __ldcg(st + 32); y.ph = __ldcg(st + 64);
+                y.pr = __ldcg(st + 96); y.pth = __ldcg(st + 128); L = __ldcg(st + 160);
+                pix = (int)__double_as_longlong(__ldcg(st + 192));
+                n_att = 0; n_acc = 0; mode = M_FRESH; loc_it = 0; on_eq = false; y_t = 0.0;
+                h_try = P.h0; h_next = P.h0; g_disk = 0.0; r_e = 0.0;
+                if (KIND == 2) {
+                    if (SPEC) {
+                        for (int k = 0; k < nf; ++k) { ACC(0, k) = 0.0; ACC(1, k) = 1.0; ACC(2, k) = 0.0; ACC(3, k) = 0.0; ACC(4, k) = 0.0; }
+                    } else {
+                        RT1(0) = 0.0; RT1(1) = 1.0; RT1(2) = 0.0; RT1(3) = 0.0; RT1(4) = 0.0;
                     }
                 }
+                if (FIFO) {
+                    sm_L[threadIdx.x] = L; LN(Q_OATT) = -1;
+                    LN(Q_LAST) = (int)(f_head - 1u); prev_out = true;   // "latest point": already processed, outside the region
+                }
+                active = true;
+            } else if (want && queue_done) {
+                exhausted = true;                                      // nothing left in the stash or in the queue
             }
+            const int served = __popc(need);
+            st_cnt = served < st_cnt ? st_cnt - served : 0;
+            __syncwarp();                                              // (the stash is rewritten only after every lane has read its entry)
         }
         const bool any_active = __any_sync(FULL, active);
         if (!any_active) {
@@ -657,24 +682,6 @@ __global__ void __launch_bounds__(128, 4) spectrum_rt_kernel(const __grid_consta
     }
     __syncthreads();
     if (O.nuLnu) for (int q = threadIdx.x; q < nf; q += blockDim.x) if (sed[q] != 0.0) atomicAdd(&O.nuLnu[q], P.sed_coef * P.nu[q] * sed[q]);
-}
-
-// Camera kernel: queue slot q -> pixel (the same 8 x 4 tile mapping as the main kernels) -> initial state and L
-// (§2.2, eqs. (18)-(26), (7), (8), (4), (5)), stored [component][slot] so that both this kernel's
-// stores and the main kernel's refill loads are contiguous per warp.  One thread per slot, every lane busy.
-__global__ void __launch_bounds__(256) init_rays_kernel(const __grid_constant__ Params P, double* __restrict__ state) {
-    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < P.n_queue; q += (long long)gridDim.x * blockDim.x) {
-        const int tile = (int)(q >> 5), w = (int)(q & 31);
-        const int i = (tile % P.tiles_x) * TILE_W + (w & (TILE_W - 1));
-        const int j = (tile / P.tiles_x) * TILE_H + (w / TILE_W);
-        if (i >= P.nx || j >= P.ny) continue;                            // slot outside a ragged image: never read
-        const double x = P.x_min + (i + 0.5) * P.x_span / P.nx;          // pixel centres (reading K)
-        const double yy = P.y_min + (j + P.row0 + 0.5) * P.y_span / P.ny_image;
-        State y; double L;
-        init_ray(P, x, yy, y, L);
-        state[q] = y.r; state[q + P.n_queue] = y.th; state[q + 2 * P.n_queue] = y.ph;
-        state[q + 3 * P.n_queue] = y.pr; state[q + 4 * P.n_queue] = y.pth; state[q + 5 * P.n_queue] = L;
-    }
 }
 
 // Diagnostic kernel behind odyssey_eval_math: the device elementary functions, elementwise.

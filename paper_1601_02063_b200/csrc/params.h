@@ -8,6 +8,7 @@ namespace ody {
 
 constexpr int MAX_FREQ = 32;
 constexpr int TILE_W = 8, TILE_H = 4;          // one queue tile = 8x4 pixels = one warp's first batch
+constexpr int STASH_DOUBLES = 7 * 32;          // per warp: the prepared rays of one queue tile (see the refill in odyssey_kernels.cuh)
 constexpr int LOCATE_MAX = 8;                  // Newton re-attempts of the event location
 constexpr int NODE_DOUBLES = 8;                // two-phase spectrum path: h, fac, E, t0, u0, ycoef, n_attempt (+ 1 pad) per node:
                                                // 64 bytes, written and read as four aligned 16-byte vectors (two whole 32-byte sectors)
@@ -74,7 +75,7 @@ struct Outputs {
     long long node_cap;                          // > 0: fixed capacity, ray's nodes start at pix * node_cap (node_offset unused)
     int32_t* overflow;                           // record pass: set to 1 when a ray needs more than node_cap nodes
     unsigned long long* queue;                   // work-queue counter (zeroed before the launch)
-    const double* init_state;                    // library scratch: initial states by queue slot, [6][n_queue] (init_rays_kernel)
+    double* stash;                               // library scratch: per warp of the grid, 32 prepared rays x 7 doubles (y, L, pixel index)
     long long image_stride;                      // spectrum_rt_kernel: elements between the images of two frequencies (0: nx * ny)
 };
 
