@@ -41,7 +41,11 @@ int fail(int code, const char* fmt, ...) {
 // (Every launch takes its work-queue counter and the warps' ray stashes from stream-ordered scratch of its own, so
 // any number of calls may be in flight on any number of streams, and a captured graph owns what it captured.)
 constexpr int MAX_DEV = 16;
-struct DevState { bool ready = false; int n_sm = 0; cudaMemPool_t pool = nullptr; };
+struct DevState {
+    bool ready = false; int n_sm = 0; cudaMemPool_t pool = nullptr;
+    cudaStream_t band_stream[2] = {nullptr, nullptr};      // the _host variants' two pipeline streams (created on first use)
+    cudaEvent_t band_event[3] = {nullptr, nullptr, nullptr};
+};
 DevState g_dev[MAX_DEV];
 std::mutex g_mu;
 
@@ -442,6 +446,66 @@ struct Scratch {
     }
 };
 #define TRY(expr) do { int rc_ = (expr); if (rc_) return rc_; } while (0)
+
+// The per-pixel work of a _host call, pipelined: the image is cut into bands of whole rows that alternate between two
+// streams; a band's device->host copies run while the next band integrates (both kernels are persistent grids, so
+// the next band's blocks move in as the previous band's finish: no idle tail between bands).  Same kernels, same
+// Params apart from the row window (row0, ny of ny_image), so every pixel is bit-identical to the one-launch result.
+// P / O describe the whole image with DEVICE pointers from S; arrays of S with `npix` elements are per-pixel.
+constexpr long long BAND_MIN_RAYS = 1 << 20;
+constexpr int BAND_MAX = 16;
+int run_host_pipelined(const Params& P, const Outputs& O, int tab, Scratch& S, size_t npix) {
+    DevState* D = nullptr;
+    TRY(device_state(&D, nullptr));
+    int nb = (int)std::min<long long>(BAND_MAX, (long long)npix / BAND_MIN_RAYS);
+    if (nb > P.ny / (2 * TILE_H)) nb = P.ny / (2 * TILE_H);
+    if (nb < 2) {                                                   // small image: one launch, then the copies
+        TRY(launch(P, O, false, tab, nullptr));
+        return S.copy_back();
+    }
+    {
+        std::lock_guard<std::mutex> lk(g_mu);
+        for (int i = 0; i < 2; ++i) if (!D->band_stream[i]) CUDA_TRY(cudaStreamCreateWithFlags(&D->band_stream[i], cudaStreamNonBlocking));
+        for (int i = 0; i < 3; ++i) if (!D->band_event[i]) CUDA_TRY(cudaEventCreateWithFlags(&D->band_event[i], cudaEventDisableTiming));
+    }
+    // the device buffers were allocated in stream 0's order
+    CUDA_TRY(cudaEventRecord(D->band_event[2], 0));
+    for (int i = 0; i < 2; ++i) CUDA_TRY(cudaStreamWaitEvent(D->band_stream[i], D->band_event[2], 0));
+    int rc = ODYSSEY_OK;
+    for (int b = 0; b < nb && rc == ODYSSEY_OK; ++b) {
+        const int j0 = (int)((long long)P.ny * b / nb) / TILE_H * TILE_H;
+        const int j1 = (b + 1 == nb) ? P.ny : (int)((long long)P.ny * (b + 1) / nb) / TILE_H * TILE_H;
+        cudaStream_t st = D->band_stream[b & 1];
+        Params Pb = P;
+        Pb.ny = j1 - j0; Pb.row0 = j0;
+        Pb.n_queue = (long long)Pb.tiles_x * ((Pb.ny + TILE_H - 1) / TILE_H) * (TILE_W * TILE_H);
+        const size_t shift = (size_t)j0 * P.nx, count = (size_t)(j1 - j0) * P.nx;
+        Outputs Ob = O;
+        if (O.flag) Ob.flag = O.flag + shift;
+        if (O.r) Ob.r = O.r + shift;
+        if (O.th) Ob.th = O.th + shift;
+        if (O.ph) Ob.ph = O.ph + shift;
+        if (O.t) Ob.t = O.t + shift;
+        if (O.n_attempt) Ob.n_attempt = O.n_attempt + shift;
+        if (O.n_accept) Ob.n_accept = O.n_accept + shift;
+        if (O.image) Ob.image = O.image + shift;
+        if (O.aux0) Ob.aux0 = O.aux0 + shift;
+        if (O.aux1) Ob.aux1 = O.aux1 + shift;
+        if (O.images) Ob.images = O.images + shift;
+        rc = launch(Pb, Ob, false, tab, st);
+        for (int i = 0; i < S.n && rc == ODYSSEY_OK; ++i) {
+            if (S.bytes[i] % npix != 0 || S.bytes[i] / npix > 8) continue;          // not a per-pixel array
+            const size_t el = S.bytes[i] / npix;
+            if (cudaMemcpyAsync((char*)S.host[i] + shift * el, (char*)S.dev[i] + shift * el, count * el, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+                rc = fail(ODYSSEY_ERR_CUDA, "device->host copy of band %d failed: %s", b, cudaGetErrorString(cudaGetLastError()));
+        }
+    }
+    // join: the host waits for both streams (also on failure: the buffers are freed in stream 0's order afterwards)
+    cudaError_t e0 = cudaStreamSynchronize(D->band_stream[0]), e1 = cudaStreamSynchronize(D->band_stream[1]);
+    if (rc == ODYSSEY_OK && (e0 != cudaSuccess || e1 != cudaSuccess))
+        rc = fail(ODYSSEY_ERR_CUDA, "pipelined render: %s", cudaGetErrorString(e0 != cudaSuccess ? e0 : e1));
+    return rc;
+}
 }  // namespace
 
 // ================================================================================================
@@ -566,8 +630,10 @@ int odyssey_trace_geodesics_host(const odyssey_scene* scene, int32_t* flag, doub
     Scratch S; int32_t *dflag, *datt, *dacc; double *dr, *dth, *dph, *dt;
     TRY(S.add(flag, n, &dflag)); TRY(S.add(r, n, &dr)); TRY(S.add(theta, n, &dth)); TRY(S.add(phi, n, &dph)); TRY(S.add(t, n, &dt));
     TRY(S.add(n_attempt, n, &datt)); TRY(S.add(n_accept, n, &dacc));
-    TRY(odyssey_trace_geodesics(scene, dflag, dr, dth, dph, dt, datt, dacc, nullptr));
-    return S.copy_back();
+    Params P; fill_params(*scene, nullptr, nullptr, 0, &P);
+    Outputs O = no_outputs();
+    O.flag = dflag; O.r = dr; O.th = dth; O.ph = dph; O.t = dt; O.n_attempt = datt; O.n_accept = dacc;
+    return run_host_pipelined(P, O, scene->tableau, S, n);
 }
 
 int odyssey_render_image_host(const odyssey_scene* scene, const odyssey_model* model, double nu_hz,
@@ -579,8 +645,16 @@ int odyssey_render_image_host(const odyssey_scene* scene, const odyssey_model* m
     TRY(S.add(image, n, &dimg)); TRY(S.add(aux0, n, &da0)); TRY(S.add(aux1, n, &da1));
     TRY(S.add(flag, n, &dflag)); TRY(S.add(n_attempt, n, &datt)); TRY(S.add(n_accept, n, &dacc));
     TRY(S.add((model->kind == ODYSSEY_KIND_THIN_DISK && model->nbins > 0) ? hist : nullptr, (size_t)model->nbins, &dhist));
-    TRY(odyssey_render_image(scene, model, nu_hz, dimg, da0, da1, dflag, datt, dacc, dhist, nullptr));
-    return S.copy_back();
+    if (dhist || model->kind == ODYSSEY_KIND_HOT_SPOT || ((model->kind == ODYSSEY_KIND_RIAF || model->kind == ODYSSEY_KIND_NT_DISK) && !(nu_hz > 0.0))) {
+        // the line histogram is a sum over the whole image (one launch); invalid arguments are reported by the device call
+        TRY(odyssey_render_image(scene, model, nu_hz, dimg, da0, da1, dflag, datt, dacc, dhist, nullptr));
+        return S.copy_back();
+    }
+    Params P; fill_params(*scene, model, &nu_hz, 1, &P);
+    Outputs O = no_outputs();
+    if (model->kind == ODYSSEY_KIND_NT_DISK) O.images = dimg;
+    O.image = dimg; O.aux0 = da0; O.aux1 = da1; O.flag = dflag; O.n_attempt = datt; O.n_accept = dacc;
+    return run_host_pipelined(P, O, scene->tableau, S, n);
 }
 
 int odyssey_render_spectrum_host(const odyssey_scene* scene, const odyssey_model* model, const double* nu_hz_host, int nf,
@@ -677,6 +751,8 @@ void odyssey_shutdown(void) {
         if (!g_dev[d].ready) continue;
         cudaSetDevice(d);
         cudaDeviceSynchronize();
+        for (int i = 0; i < 2; ++i) if (g_dev[d].band_stream[i]) cudaStreamDestroy(g_dev[d].band_stream[i]);
+        for (int i = 0; i < 3; ++i) if (g_dev[d].band_event[i]) cudaEventDestroy(g_dev[d].band_event[i]);
         if (g_dev[d].pool) cudaMemPoolDestroy(g_dev[d].pool);
         g_dev[d] = DevState();
     }

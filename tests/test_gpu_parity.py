@@ -141,6 +141,47 @@ def test_host_entry_points_match_device_entry_points(ody):
     assert np.allclose(_np(s["nuLnu"]), sh["nuLnu"], rtol=1e-12)
 
 
+def test_pipelined_host_call_is_bit_identical_to_the_device_call(ody):
+    """Images of 2^21 pixels and more go through the _host variants in bands of rows on two streams, the
+    device->host copy of a band overlapping the next band's kernel: every array must equal the one-launch
+    device result bit for bit (same kernels, same constants, only the row window differs)."""
+    w = W.C2(n=1536)
+    sc = dict(w["scene"], ny=1404)                        # 2 156 544 pixels: two bands, the second one ragged (1404 = 351 x 4)
+    dev = ody.render_image(sc, w["model"], w["nu"][0]); _sync()
+    host = ody.render_image_host(sc, w["model"], w["nu"][0])
+    for k in ("image", "aux0", "aux1", "flag", "n_attempt", "n_accept"):
+        assert np.array_equal(_np(dev[k]), host[k]), k
+    g = ody.trace_geodesics(sc, with_time=True); _sync()
+    gh = ody.trace_geodesics_host(sc, with_time=True)
+    for k in g:
+        assert np.array_equal(_np(g[k]), gh[k]), k
+
+
+def test_one_long_call_against_many_short_calls_on_other_streams(ody):
+    """Every launch owns its work-queue counter (stream-ordered scratch): a long render on one stream is not
+    disturbed by 70 short calls issued meanwhile on 70 other streams (the first version handed out counters from
+    a ring of 64 and the 65th launch zeroed the first one's)."""
+    import torch
+    big, small = W.C2(n=768), W.C0(n=24)
+    ref_big = {k: _np(v).copy() for k, v in ody.render_image(big["scene"], big["model"], big["nu"][0]).items() if v is not None}
+    ref_small = {k: _np(v).copy() for k, v in ody.trace_geodesics(small["scene"]).items()}
+    _sync()
+    s_big = torch.cuda.Stream()
+    streams = [torch.cuda.Stream() for _ in range(70)]
+    with torch.cuda.stream(s_big):
+        out_big = ody.render_image(big["scene"], big["model"], big["nu"][0])
+    outs = []
+    for s in streams:
+        with torch.cuda.stream(s):
+            outs.append(ody.trace_geodesics(small["scene"]))
+    _sync()
+    for k, v in ref_big.items():
+        assert np.array_equal(_np(out_big[k]), v), f"long call: {k} disturbed"
+    for o in outs:
+        for k, v in ref_small.items():
+            assert np.array_equal(_np(o[k]), v), f"short call: {k} wrong"
+
+
 def test_concurrent_calls_on_different_streams_do_not_interfere(ody):
     """Each launch takes its own work-queue counter and passes its constants as kernel parameters, so calls
     enqueued on different streams may overlap freely."""
