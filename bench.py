@@ -35,21 +35,24 @@ import workloads as W  # noqa: E402
 METRIC = "ns per photon per RK step (FP64)"
 UNIT = "ns/photon/step"
 
-# FP64 work per unit: flop per attempted RK step of the geodesic system, and per
-# radiative-transfer update (one per accepted step, single frequency).  These are flop the kernels
-# EXECUTE (2 x DFMA + DMUL + DADD thread instructions, predicated on), measured with ncu on this very
-# workload: geodesics-only kernel 945.0 per attempt (profiles/r01_c4_geodesic_kernel_ncu_full.md); for the
-# transfer update the LEANEST build measured is used — 397.3 per update ((1262.0 - 946.6)/0.7938, the build
-# before the K_2 branches were replaced by evaluate-both-and-select) — not the 439.8 the final kernel
-# executes (profiles/r01_c4_riaf_kernel_ncu_full.md: 1294.1 per attempt), because the difference is work
-# done only to avoid a divergent branch.  SURVEY.md §8(d)'s a-priori hand count (1500 + ~490) is 58 % higher
-# still: it would overstate the achieved rate, so it is not used.
-FLOP_PER_ATTEMPT_GEODESIC = 945.0
-FLOP_PER_RT_UPDATE = 397.3
-# DRAM traffic of one launch of the fused kernel on the default workload (C4 at 4096^2), from the same ncu
-# capture: dram__bytes_read.sum + dram__bytes_write.sum = 842.4 MB + 583.5 MB (805 MB of initial states read,
-# 604 MB of outputs written).  Reported only for that workload.
-DRAM_BYTES_PER_LAUNCH_C4_4096 = 839.323904e6 + 581.184000e6
+# FP64 work per unit: flop per attempted RK step of the geodesic system and per radiative-transfer
+# update (one per accepted step, single frequency).  These are flop the kernels EXECUTE (2 x DFMA + DMUL + DADD
+# thread instructions, predicated on), counted by ncu on this very workload and kept, with the DRAM traffic, the
+# warp execution efficiency and the FP64-pipe utilisation of the same captures, in profiles/r02_flop_counts.json
+# (written by bench_counts.py; the file carries a hash of the kernel sources and the line says "stale" when the
+# sources have changed since).  SURVEY.md §8(d)'s a-priori hand count (~1500 flop per attempt + ~490 per update)
+# is reported beside it as `frac_hand_count`: it is what a straightforward implementation would execute, ~60 %
+# more than these kernels do, so it flatters the rate and is NOT the headline fraction.
+COUNTS_FILE = os.path.join(ROOT, "profiles", "r02_flop_counts.json")
+HAND_FLOP_PER_ATTEMPT, HAND_FLOP_PER_RT_UPDATE = 1500.0, 490.0
+
+
+def load_counts():
+    import bench_counts
+    with open(COUNTS_FILE) as f:
+        c = json.load(f)
+    c["stale"] = c.get("source_hash") != bench_counts.source_hash()
+    return c
 
 
 def parse_args():
@@ -66,6 +69,7 @@ def parse_args():
     p.add_argument("--no-cpu-baseline", action="store_true")
     p.add_argument("--no-e2e", action="store_true")
     p.add_argument("--no-fp32-variant", action="store_true")
+    p.add_argument("--no-extra", action="store_true", help="skip the extra.configs block (C0-C3 and the C4 sweep)")
     p.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
                    help="mixed: time the mixed-precision transfer variant as the main kernel (for ncu captures)")
     return p.parse_args()
@@ -218,6 +222,39 @@ def headline(total_ms_max, steps, attempts_all, accepts_all, world):
 
 
 # ---------------------------------------------------------------------------------------------------
+# extra.configs: device time of every BASELINE.json configuration and of the C4 sweep (outside the headline's
+# timed region; CUDA events on the launching stream, one warm-up, median of 3)
+# ---------------------------------------------------------------------------------------------------
+def time_extra_configs(ody, torch):
+    def timed(call, photons):
+        out = call(); torch.cuda.synchronize()
+        ms = []
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); out = call(); e1.record(); torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        ms.sort()
+        att = int(out["n_attempt"].sum(dtype=torch.int64).item())
+        return {"photons": photons, "ms": ms[1], "attempts": att, "ns_per_photon_step": ms[1] * 1e6 / att,
+                "images_per_s": 1e3 / ms[1]}
+
+    res = {}
+    w = W.C0(); res["C0"] = timed(lambda: ody.trace_geodesics(w["scene"]), w["scene"]["nx"] * w["scene"]["ny"])
+    w1 = W.C1(); res["C1"] = timed(lambda: ody.render_image(w1["scene"], w1["model"]), w1["scene"]["nx"] * w1["scene"]["ny"])
+    w2 = W.C2(); res["C2"] = timed(lambda: ody.render_image(w2["scene"], w2["model"], w2["nu"][0]), w2["scene"]["nx"] * w2["scene"]["ny"])
+    w3 = W.C3(); res["C3"] = dict(timed(lambda: ody.render_spectrum(w3["scene"], w3["model"], w3["nu"]), w3["scene"]["nx"] * w3["scene"]["ny"]),
+                                  frequencies=len(w3["nu"]))
+    m_rk = dict(w2["model"], rt_scheme=W.RT_RK_COMPONENTS)
+    res["C2 rt_scheme=RK components"] = timed(lambda: ody.render_image(w2["scene"], m_rk, w2["nu"][0]), w2["scene"]["nx"] * w2["scene"]["ny"])
+    for a in (0.0, 0.5, 0.9, 0.998):
+        for n in (1024, 2048, 4096):
+            w4 = W.C4(n=n, a=a)
+            res[f"C4 a={a:g} n={n}"] = timed(lambda: ody.render_image(w4["scene"], w4["model"], w4["nu"][0]), n * n)
+            torch.cuda.empty_cache()
+    return res
+
+
+# ---------------------------------------------------------------------------------------------------
 # the B200 arm
 # ---------------------------------------------------------------------------------------------------
 def run_b200(args):
@@ -329,7 +366,7 @@ def run_b200(args):
         torch.cuda.synchronize()
         e2e_s = time.perf_counter() - t0
         d2h = sum(v.nbytes for v in host.values() if v is not None)
-        h2d = 120 + 136 + 8                                           # the two structs and nu_hz (kernel parameters)
+        h2d = 120 + 184 + 8                                           # the two structs and nu_hz (kernel parameters)
         e2e = (e2e_s, d2h, h2d, int(host["n_attempt"].astype("int64").sum()))
 
     # ---- reduce over ranks: time = max, work = sum
@@ -342,10 +379,15 @@ def run_b200(args):
 
     head = headline(total_ms_max, args.steps, attempts_all, accepts_all, world)
     ms_per_step, value = head["ms_per_step"], head["value"]
-    flop_rt = FLOP_PER_RT_UPDATE if args.model == "riaf" else 0.0
-    flop_step = FLOP_PER_ATTEMPT_GEODESIC * attempts + flop_rt * accepts                # per launch (this rank)
+    counts = load_counts()
+    flop_geo = counts["flop_per_attempt_geodesic"]
+    flop_rt = counts["flop_per_rt_update"] if args.model == "riaf" else 0.0
+    flop_step = flop_geo * attempts + flop_rt * accepts                                # per launch (this rank)
     kernel_ms = sum(step_ms) / len(step_ms)
     achieved = flop_step / (kernel_ms * 1e-3) / 1e12
+    hand = (HAND_FLOP_PER_ATTEMPT * attempts + (HAND_FLOP_PER_RT_UPDATE if args.model == "riaf" else 0.0) * accepts) / (kernel_ms * 1e-3) / 1e12
+    cap = counts["fused_kernel" if args.model == "riaf" else "geodesic_kernel"]
+    headline_workload = args.n == 4096 and args.a == 0.998
     info = ody.kernel_info(mo["kind"], False, sc["tableau"])
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -361,10 +403,19 @@ def run_b200(args):
         "ns_per_photon_per_accepted_step": head["ns_per_photon_per_accepted_step"],
         "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                      "frac": achieved / peak_tflops,
-                     "traffic": DRAM_BYTES_PER_LAUNCH_C4_4096 if (args.model == "riaf" and args.n == 4096 and args.a == 0.998) else None,
-                     "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_c4_riaf_kernel_ncu_full.md)",
-                     "kernel": "odyssey_kernel<KIND=%d,TAB=0,SPEC=false>" % mo["kind"], "kernel_ms": kernel_ms,
-                     "flop_per_attempt": FLOP_PER_ATTEMPT_GEODESIC, "flop_per_rt_update": flop_rt,
+                     "what": "EXECUTED FP64 flop (2 x DFMA + DMUL + DADD thread instructions, ncu) / CUDA-event kernel time / DFMA peak",
+                     "traffic": cap["dram_bytes"] if headline_workload else None,
+                     "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
+                     "kernel": cap["kernel"], "kernel_ms": kernel_ms,
+                     "flop_per_attempt": flop_geo, "flop_per_rt_update": flop_rt,
+                     "counts_file": os.path.relpath(COUNTS_FILE, ROOT), "counts_source_hash": counts["source_hash"],
+                     "stale": bool(counts["stale"]),
+                     "warp_execution_efficiency": cap["warp_execution_efficiency"],
+                     "fp64_pipe_utilisation": cap["fp64_pipe_utilisation"],
+                     "fp64_share_of_warp_instructions": cap["fp64_share_of_warp_instructions"],
+                     "spill_bytes": info["local_bytes"], "local_load_store_instructions_executed": cap["local_load_store_instructions"],
+                     "frac_hand_count": hand / peak_tflops,
+                     "hand_count": "SURVEY.md 8(d) a-priori count, 1500 flop per attempt + 490 per transfer update: context, not the headline",
                      "peak_source": "odyssey_fp64_peak_probe (DFMA microbenchmark) in this run, best of 5"},
         "kernel_info": info,
         "gpu_launches": int(launches_all),
@@ -384,6 +435,10 @@ def run_b200(args):
                        "ms_per_step": e2e_s_max / args.steps * 1e3,
                        "api": "odyssey_render_image_host (pinned host buffers; device scratch, kernel and D2H copies "
                               "of all six output arrays inside the timed region)"}
+    if not args.no_extra and world == 1:
+        line["extra"] = {"configs": time_extra_configs(ody, torch),
+                         "note": "device time per call, CUDA events, median of 3 after one warm-up, outside the headline's timed region; "
+                                 "C3 = 32 frequencies per photon-step (two-phase spectrum path); BASELINE.json:configs[0..4]"}
     if not args.no_cpu_baseline and world == 1:                       # the oracle leg runs at N = 1 only
         from oracle import build as oracle_build
         oracle_build.build()

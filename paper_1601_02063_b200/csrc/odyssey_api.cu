@@ -238,7 +238,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
 #define ODY_MINB_MAIN 5                         // (-DODY_MINB_MAIN=4 builds the 128-register variant of the occupancy comparison in DESIGN.md)
 #endif
 constexpr int NT_MAIN = 128, MINB_MAIN = ODY_MINB_MAIN;     // 96 registers per thread at most
-constexpr int MINB_SPOT = 4;                    // hot spot (kind 3, with the coordinate time) and Novikov-Thorne disk (kind 4): 4 blocks per SM keep them free of spills
+constexpr int MINB_SPOT = 4;                    // thin disk, hot spot, Novikov-Thorne disk and the coordinate-time variant: 4 blocks per SM keep them free of spills
 constexpr int MINB_RK = 2;                      // transfer scheme E' (RK components): the in-loop transfer code wants > 168 registers
 constexpr int NT_SPEC = 128, MINB_SPEC = 3;     // 168 registers (the unrolled frequency loop wants them); per-frequency accumulators in a global scratch buffer
 
@@ -250,7 +250,7 @@ KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0, int prec = 0, bo
     if (kind == 4)
         return tab ? odyssey_kernel<4, 1, false, NT_MAIN, MINB_SPOT> : odyssey_kernel<4, 0, false, NT_MAIN, MINB_SPOT>;
     if (kind == 0 && time)
-        return tab ? odyssey_kernel<0, 1, false, NT_MAIN, MINB_MAIN, 0, 0, 1> : odyssey_kernel<0, 0, false, NT_MAIN, MINB_MAIN, 0, 0, 1>;
+        return tab ? odyssey_kernel<0, 1, false, NT_MAIN, MINB_SPOT, 0, 0, 1> : odyssey_kernel<0, 0, false, NT_MAIN, MINB_SPOT, 0, 0, 1>;
     if (kind == 2 && !spec && rts == 0 && prec == 1)
         return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_MAIN, 0, 1> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_MAIN, 0, 1>;
     if (kind == 2 && !spec && rts == 1)
@@ -262,7 +262,7 @@ KernelFn pick_kernel(int kind, bool spec, int tab, int rts = 0, int prec = 0, bo
     if (spec) return tab ? odyssey_kernel<2, 1, true, NT_SPEC, MINB_SPEC> : odyssey_kernel<2, 0, true, NT_SPEC, MINB_SPEC>;
     switch (kind) {
         case 0: return tab ? odyssey_kernel<0, 1, false, NT_MAIN, MINB_MAIN> : odyssey_kernel<0, 0, false, NT_MAIN, MINB_MAIN>;
-        case 1: return tab ? odyssey_kernel<1, 1, false, NT_MAIN, MINB_MAIN> : odyssey_kernel<1, 0, false, NT_MAIN, MINB_MAIN>;
+        case 1: return tab ? odyssey_kernel<1, 1, false, NT_MAIN, MINB_SPOT> : odyssey_kernel<1, 0, false, NT_MAIN, MINB_SPOT>;
         default: return tab ? odyssey_kernel<2, 1, false, NT_MAIN, MINB_MAIN> : odyssey_kernel<2, 0, false, NT_MAIN, MINB_MAIN>;
     }
 }

@@ -67,10 +67,10 @@ __host__ __device__ constexpr int smem_per_thread(int rts) { return (rts == 1 ? 
 #define ODY_RT_FIFO 1
 #endif
 constexpr int FIFO_CAP = 64;
-constexpr int FIFO_DOUBLES = 7 * FIFO_CAP;                               // per warp
+constexpr int FIFO_DOUBLES = 5 * FIFO_CAP + 3 * FIFO_CAP / 2;               // per warp: 5 doubles + 3 ints per point
 constexpr int FIFO_ACC_BITS = 25;                                        // accepted-step counts below 2^25 (check_scene)
 __host__ __device__ constexpr bool uses_fifo(int kind, bool spec, int rts) { return ODY_RT_FIFO && kind == 2 && !spec && rts == 0; }
-__host__ __device__ constexpr int fifo_doubles_per_block(int nt) { return nt + (nt / 32) * FIFO_DOUBLES + 2 * nt; }
+__host__ __device__ constexpr int fifo_doubles_per_block(int nt) { return nt + (nt / 32) * FIFO_DOUBLES + 3 * nt + 2 * nt; }   // L, rings, 6 ints per thread, next step length and φ slope
 
 // RTS = 1: transfer scheme E' (tau, I as Runge–Kutta components; single frequency only).
 // RTS = 2: record mode, the first phase of the two-phase spectrum path (see spectrum_rt_kernel below).
@@ -103,30 +103,38 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     constexpr bool FIFO = uses_fifo(KIND, SPEC, RTS);
     double* const sm_L = sm_red;                                                          // [NT] L of the lane's ray
     double* const sm_ring = sm_red + NT + (threadIdx.x >> 5) * FIFO_DOUBLES;              // this warp's ring
-    int4* const sm_ringi = reinterpret_cast<int4*>(sm_ring + 5 * FIFO_CAP);
-    int* const sm_lane = reinterpret_cast<int*>(sm_red + NT + (NT / 32) * FIFO_DOUBLES);  // [4][NT] ints, see the Q_ indices
-    constexpr int Q_OATT = 0, Q_OACC = 1, Q_LAST = 2, Q_END = 3;                          // opaque crossing: n_attempt (-1: none), n_accept; latest ring position; end flag
+    int* const sm_ringi = reinterpret_cast<int*>(sm_ring + 5 * FIFO_CAP);                // [3][FIFO_CAP]: n_attempt, packed n_accept, previous position
+    int* const sm_lane = reinterpret_cast<int*>(sm_red + NT + (NT / 32) * FIFO_DOUBLES);  // [6][NT] ints, see the Q_ indices
+    double* const sm_hnext = sm_red + NT + (NT / 32) * FIFO_DOUBLES + 3 * NT;             // [2][NT]: next step length, φ slope of the first stage
+    constexpr int Q_OATT = 0, Q_OACC = 1, Q_LAST = 2, Q_END = 3, Q_PIX = 4, Q_NACC = 5;                          // opaque crossing: n_attempt (-1: none), n_accept; latest ring position; end flag
     double* const sm_rtw = smem + (smem_per_thread(RTS) - 5) * NT + (threadIdx.x & ~31);  // RT state of this warp's lane 0
 #define FD(f, slot) sm_ring[(f) * FIFO_CAP + (slot)]
 #define LN(q) sm_lane[(q) * NT + threadIdx.x]
     unsigned f_head = 0, f_tail = 0;                                                      // ring positions (warp-uniform)
     int drain_wait = 0;
-    bool draining = false, prev_out = true;
 
     // the warp's stash of prepared rays (see the refill): [7][32] doubles of scratch
     double* const stash = O.stash + ((size_t)blockIdx.x * (NT / 32) + (threadIdx.x >> 5)) * STASH_DOUBLES;
-    int st_cnt = 0;                                                                       // prepared rays left (warp-uniform)
-    bool queue_done = false;                                                              // the queue has handed out its last tile
+    int st_w = 0;                          // warp-uniform: prepared rays left (bits 0..5) | 64 once the queue has handed out its last tile
 
     const double a = P.a, a2 = P.a2;
-    bool active = false, exhausted = false, on_eq = false;
-    int pix = 0, n_att = 0, n_acc = 0, mode = M_NORMAL, loc_it = 0;
+    // the lane's status bits share one register
+    struct { unsigned active : 1, exhausted : 1, on_eq : 1, draining : 1, prev_out : 1; } B;
+    B.active = 0; B.exhausted = 0; B.on_eq = 0; B.draining = 0; B.prev_out = 1;
+    // (FIFO kernel: the pixel index, the accepted-step count and the next step length — each touched once per trip at
+    // most — live in shared memory; at 96 registers the compiler would otherwise spill them to local memory)
+    int pix_reg = 0, n_acc_reg = 0, n_att = 0, mode = M_NORMAL, loc_it = 0;
+    double h_next_reg = 0.0;
+    int& pix = FIFO ? sm_lane[Q_PIX * NT + threadIdx.x] : pix_reg;
+    int& n_acc = FIFO ? sm_lane[Q_NACC * NT + threadIdx.x] : n_acc_reg;
+    double& h_next = FIFO ? sm_hnext[threadIdx.x] : h_next_reg;
     State y;
     StagesSmem<NT> K;
     K.base = smem + threadIdx.x;
-    double kph0 = 0.0;                                              // φ slope of the cached first stage
+    double kph0_reg = 0.0;                                          // φ slope of the cached first stage
+    double& kph0 = FIFO ? sm_hnext[NT + threadIdx.x] : kph0_reg;
     double y_t = 0.0, kt0 = 0.0;                                    // (TIME) coordinate time and its cached first slope
-    double L = 0.0, h_try = 0.0, h_next = 0.0, cos_y = 0.0;
+    double L = 0.0, h_try = 0.0, cos_y = 0.0;
     double g_disk = 0.0, r_e = 0.0;
     y.r = y.th = y.ph = y.pr = y.pth = 0.0;
 #pragma unroll
@@ -144,8 +152,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         const bool have = lane < nb;
         const int slot = (int)((f_head + lane) & (FIFO_CAP - 1));
         double er = 0.0, esn = 0.0, ecn = 0.0, epr = 0.0, eh = 0.0;
-        int4 meta = make_int4(0, 0, 0, 0);
-        if (have) { er = FD(0, slot); esn = FD(1, slot); ecn = FD(2, slot); epr = FD(3, slot); eh = FD(4, slot); meta = sm_ringi[slot]; }
+        int3 meta = make_int3(0, 0, 0);
+        if (have) { er = FD(0, slot); esn = FD(1, slot); ecn = FD(2, slot); epr = FD(3, slot); eh = FD(4, slot); meta = make_int3(sm_ringi[slot], sm_ringi[FIFO_CAP + slot], sm_ringi[2 * FIFO_CAP + slot]); }
         const int o = (meta.y >> FIFO_ACC_BITS) & 31;
         double a1 = 0.0, e1 = 0.0;
         if (have) {
@@ -186,7 +194,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     };
     // ---- a ray whose points have all been processed: outputs (kind 2, single frequency), the lane is free again
     auto fifo_finalize = [&]() {
-        if (draining && (int)(f_head - (unsigned)LN(Q_LAST)) > 0) {
+        if (B.draining && (int)(f_head - (unsigned)LN(Q_LAST)) > 0) {
             int oflag = LN(Q_END), oatt = n_att, oacc = n_acc;
             if (LN(Q_OATT) >= 0) { oflag = F_OPAQUE; oatt = LN(Q_OATT); oacc = LN(Q_OACC); }
             if (O.flag) O.flag[pix] = oflag;
@@ -195,7 +203,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             if (O.image) O.image[pix] = P.nu3[0] * RT1(2);
             if (O.aux0) O.aux0[pix] = RT1(0);
             if (O.aux1) O.aux1[pix] = 0.0;
-            draining = false;
+            B.draining = false;
         }
     };
 
@@ -208,14 +216,13 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         // not, builds the state of one of its pixels.  The stash is 32 x 7 doubles per warp of stream-ordered
         // scratch (a few MB for the whole grid: it lives in L2), so there is no camera kernel, no per-pixel
         // scratch and no HBM traffic beyond the outputs.
-        const bool want = !active && !exhausted && !(FIFO && draining);
+        const bool want = !B.active && !B.exhausted && !(FIFO && B.draining);
         const unsigned need = __ballot_sync(FULL, want);
         if (need) {
-            if (st_cnt == 0 && !queue_done) {
+            if (st_w == 0) {                                           // stash empty, queue not finished
                 unsigned long long base = 0;
                 if (lane == 0) base = atomicAdd(O.queue, 32ull);
                 base = __shfl_sync(FULL, base, 0);
-                queue_done = (long long)base + 32 >= P.n_queue;
                 const long long q = (long long)base + lane;
                 const int tile = (int)(q >> 5), w = (int)(q & 31);
                 const int i = (tile % P.tiles_x) * TILE_W + (w & (TILE_W - 1));
@@ -231,16 +238,17 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     stash[idx] = y0.r; stash[32 + idx] = y0.th; stash[64 + idx] = y0.ph; stash[96 + idx] = y0.pr;
                     stash[128 + idx] = y0.pth; stash[160 + idx] = L0; stash[192 + idx] = __longlong_as_double((long long)(j * P.nx + i));
                 }
-                st_cnt = __popc(vm);
+                st_w = __popc(vm) | ((long long)base + 32 >= P.n_queue ? 64 : 0);
                 __syncwarp();
             }
             const int rank = __popc(need & ((1u << lane) - 1u));
+            const int st_cnt = st_w & 63;
             if (want && rank < st_cnt) {
                 const double* st = stash + (st_cnt - 1 - rank);
                 y.r = __ldcg(st); y.th = __ldcg(st + 32); y.ph = __ldcg(st + 64);
                 y.pr = __ldcg(st + 96); y.pth = __ldcg(st + 128); L = __ldcg(st + 160);
                 pix = (int)__double_as_longlong(__ldcg(st + 192));
-                n_att = 0; n_acc = 0; mode = M_FRESH; loc_it = 0; on_eq = false; y_t = 0.0;
+                n_att = 0; n_acc = 0; mode = M_FRESH; loc_it = 0; B.on_eq = false; y_t = 0.0;
                 h_try = P.h0; h_next = P.h0; g_disk = 0.0; r_e = 0.0;
                 if (KIND == 2) {
                     if (SPEC) {
@@ -251,30 +259,30 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                 }
                 if (FIFO) {
                     sm_L[threadIdx.x] = L; LN(Q_OATT) = -1;
-                    LN(Q_LAST) = (int)(f_head - 1u); prev_out = true;   // "latest point": already processed, outside the region
+                    LN(Q_LAST) = (int)(f_head - 1u); B.prev_out = true;   // "latest point": already processed, outside the region
                 }
-                active = true;
-            } else if (want && queue_done) {
-                exhausted = true;                                      // nothing left in the stash or in the queue
+                B.active = true;
+            } else if (want && (st_w & 64)) {
+                B.exhausted = true;                                      // nothing left in the stash or in the queue
             }
             const int served = __popc(need);
-            st_cnt = served < st_cnt ? st_cnt - served : 0;
+            st_w = (st_w & 64) | (served < st_cnt ? st_cnt - served : 0);
             __syncwarp();                                              // (the stash is rewritten only after every lane has read its entry)
         }
-        const bool any_active = __any_sync(FULL, active);
+        const bool any_active = __any_sync(FULL, B.active);
         if (!any_active) {
             // (FIFO) no ray running but points waiting or lanes draining: fall through — the attempt below runs with every
             // lane off (this happens only at the very end of the image), the ring is flushed, the drained lanes released
-            if (!(FIFO && (f_tail != f_head || __any_sync(FULL, draining)))) {
-                if (__all_sync(FULL, exhausted)) break;
+            if (!(FIFO && (f_tail != f_head || __any_sync(FULL, B.draining)))) {
+                if (__all_sync(FULL, B.exhausted)) break;
                 continue;
             }
         }
 
         // ------------------------------------------------------------------ one attempt
         int flag = -1;
-        const bool fresh = active && mode == M_FRESH;
-        bool run = active && !fresh;                                   // takes part in stages 2..6
+        const bool fresh = B.active && mode == M_FRESH;
+        bool run = B.active && !fresh;                                   // takes part in stages 2..6
         if (run && mode == M_NORMAL && n_att >= P.max_attempts) { flag = F_MAXSTEP; run = false; }
         bool done = false;                                             // end state evaluated: go on to events / commit
         double ph5 = kRkB5[TAB][0] * kph0;
@@ -347,8 +355,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             if (mode == M_NORMAL) {                                    // fresh accepted step: detect events
                 int m = M_NORMAL;
                 if (KIND == 1 || KIND == 3 || KIND == 4) {
-                    if (!on_eq && cos_y * cn < 0.0) m = M_EQ;          // equatorial crossing (reading P)
-                    else on_eq = false;
+                    if (!B.on_eq && cos_y * cn < 0.0) m = M_EQ;          // equatorial crossing (reading P)
+                    else B.on_eq = false;
                 }
                 if (m == M_NORMAL) m = radial_event(P, yn);
                 mode = m; loc_it = 0;
@@ -367,7 +375,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     break;
                 }
                 if (mode == M_EQ) {
-                    on_eq = true; mode = M_NORMAL;
+                    B.on_eq = true; mode = M_NORMAL;
                     if (yn.r >= P.r_in && yn.r <= P.r_out && yn.r > P.r_cap) {
                         flag = F_DISK; r_e = yn.r;
                         double igam;
@@ -413,14 +421,16 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             const bool step_pt = commit || fresh;
             const bool inside = yn.r > P.r_cap && yn.r < P.r_rt_out;
             // a point outside the emitting region whose predecessor was outside too contributes nothing
-            const bool push = step_pt && (inside || !prev_out || P.tau_max < 0.0);
+            const bool push = step_pt && (inside || !B.prev_out || P.tau_max < 0.0);
             const unsigned pm = __ballot_sync(FULL, push);
             if (push) {
                 const unsigned pos = f_tail + __popc(pm & ((1u << lane) - 1u));
                 const int slot = (int)(pos & (FIFO_CAP - 1));
                 FD(0, slot) = yn.r; FD(1, slot) = sn; FD(2, slot) = cn; FD(3, slot) = yn.pr; FD(4, slot) = commit ? h_try : 0.0;
-                sm_ringi[slot] = make_int4(n_att, n_acc | (lane << FIFO_ACC_BITS) | (flag >= 0 ? 1 << 30 : 0) | (commit ? 1 << 31 : 0), LN(Q_LAST), 0);
-                LN(Q_LAST) = (int)pos; prev_out = !inside;
+                sm_ringi[slot] = n_att;
+                sm_ringi[FIFO_CAP + slot] = n_acc | (lane << FIFO_ACC_BITS) | (flag >= 0 ? 1 << 30 : 0) | (commit ? 1 << 31 : 0);
+                sm_ringi[2 * FIFO_CAP + slot] = LN(Q_LAST);
+                LN(Q_LAST) = (int)pos; B.prev_out = !inside;
             }
             f_tail += __popc(pm);
             __syncwarp();
@@ -472,10 +482,10 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
 
         // ------------------------------------------------------------------ ray ended: outputs, release the lane
         if (FIFO) {
-            if (active && flag < 0 && LN(Q_OATT) >= 0) flag = F_OPAQUE;                 // found opaque by the ring: stop here
-            if (active && flag >= 0) { active = false; draining = true; LN(Q_END) = flag; }
+            if (B.active && flag < 0 && LN(Q_OATT) >= 0) flag = F_OPAQUE;                 // found opaque by the ring: stop here
+            if (B.active && flag >= 0) { B.active = false; B.draining = true; LN(Q_END) = flag; }
             fifo_finalize();
-            drain_wait = __any_sync(FULL, draining) ? drain_wait + 1 : 0;
+            drain_wait = __any_sync(FULL, B.draining) ? drain_wait + 1 : 0;
         } else if (flag >= 0) {
             if (O.flag) O.flag[pix] = flag;
             if (O.r) O.r[pix] = y.r;
@@ -558,7 +568,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     if (O.nuLnu) atomicAdd(&sm_red[k], v);
                 }
             }
-            active = false;
+            B.active = false;
         }
     }
 #undef ACC
