@@ -27,10 +27,14 @@
 // 8-component scipy integration of Hamilton's equations (E, L_z drift there); closed-form Keplerian
 // g; uniform-slab RT; the thin limit and the formal solution int eps e^-tau dlambda by independent
 // quadrature on a finer path; K_2 vs scipy; M(1) as printed in eq. (38).
-// PARITY UNPINNED: the RIAF images and the SED as a whole (oracle_render_image kind 2,
-// oracle_render_spectrum) have no value printed in the paper to compare with (Figs. 9, 10 are
-// pictures, Broderick & Loeb's table is not in the container); their parts are pinned, the whole
-// only by convergence under rtol refinement.
+// The RIAF images and the SED as a whole (oracle_render_image kind 2, oracle_render_spectrum) have no value
+// printed in the paper to compare with (Figs. 9, 10 are pictures, Broderick & Loeb's table is not in the
+// container); they are pinned end to end by tests/test_oracle_riaf_independent.py against a computation that
+// shares nothing with this file (tests/riaf_reference.py: momenta from the metric and the null condition, scipy
+// DOP853 on the symbolically derived 8-component Hamiltonian system with eqs. (30), (31) as two more components,
+// scipy's K_2): pixels of C2 thin and thick, captured, escaping and frozen, to the truncation level of reading E
+// (3e-3 at rtol 1e-8, converging: 6e-5 at 1e-12), a five-frequency SED, and a scene whose first and event-
+// located last step carry weight.
 //
 // Build: g++ -std=c++17 -O2 -fopenmp -fPIC -shared (see oracle/build.py).  -ffast-math is never used.
 

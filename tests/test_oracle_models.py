@@ -281,8 +281,8 @@ def test_rt_along_ray_with_absorption_equals_formal_solution_on_a_fine_path():
 
 
 def test_riaf_image_converges_under_rtol_refinement():
-    """The RIAF image as a whole has no value printed in the paper (parity unpinned): what can be checked
-    is that it converges as the step tolerance is refined — successive differences shrink."""
+    """The RIAF image as a whole has no value printed in the paper (its end-to-end pin is
+    tests/test_oracle_riaf_independent.py); here: it converges as the step tolerance is refined."""
     w = W.C2(n=20)
     imgs = []
     for rtol in (1e-6, 1e-8, 1e-10):
