@@ -160,17 +160,46 @@ def test_c4_sweep_spins_sampled_at_1024(ody, orc, a):
     _check_image(_sub(_np(out["image"]), idx), ref["image"], f"C4 a={a}")
 
 
-def test_c4_full_size_sampled(ody, orc):
-    """4096 x 4096, the exact launch bench.py times."""
-    w = W.C4()
+@pytest.mark.parametrize("a", [0.5, 0.998])
+def test_c4_sweep_sampled_at_2048(ody, orc, a):
+    w = W.C4(n=2048, a=a)
     out = ody.render_image(w["scene"], w["model"], w["nu"][0]); _sync()
-    idx = W.subgrid_indices(w["scene"], 64)
+    idx = W.subgrid_indices(w["scene"], 96)
     ref = orc.render_image(w["scene"], w["model"], w["nu"][0], idx=idx)
     assert np.array_equal(_sub(_np(out["flag"]), idx), ref["flag"])
+    _check_image(_sub(_np(out["image"]), idx), ref["image"], f"C4 2048^2 a={a}")
+    assert np.mean(_sub(_np(out["n_attempt"]), idx) == ref["n_attempt"]) >= 0.995
+    img = _np(out["image"])
+    assert np.all(np.isfinite(img)) and img.min() >= 0.0
+
+
+def test_c4_full_size_sampled(ody, orc):
+    """4096 x 4096, the exact launch bench.py times: a 128 x 128 grid over the whole frame plus every 8th pixel in both
+    directions of the window |x| < 8, |y| < 7 that holds the shadow and the photon ring (81 920 pixels in all,
+    each computed by the oracle), and the whole frame finite, non-negative, every pixel written."""
+    w = W.C4()
+    sc = w["scene"]
+    out = ody.render_image(sc, w["model"], w["nu"][0]); _sync()
+    ii, jj = W.subgrid_indices(sc, 128)
+    n, half = sc["nx"], sc["x_max"]
+    lo = lambda v: int((v + half) / (2 * half) * n)
+    for j in range(lo(-7.0), lo(7.0), 8):
+        for i in range(lo(-8.0), lo(8.0), 8):
+            ii.append(i); jj.append(j)
+    idx = (ii, jj)
+    assert len(ii) >= 256 * 256
+    ref = orc.render_image(sc, w["model"], w["nu"][0], idx=idx)
+    assert np.array_equal(_sub(_np(out["flag"]), idx), ref["flag"])
+    assert {W.FLAG_CAPTURED, W.FLAG_ESCAPED} <= set(np.unique(ref["flag"]))
     _check_image(_sub(_np(out["image"]), idx), ref["image"], "C4 4096^2 sampled")
+    assert ref["n_attempt"].max() > 400                                  # the sample reaches the long, winding rays of the ring
     n_att = _np(out["n_attempt"])
-    assert n_att.min() > 0 and n_att.max() < w["scene"]["max_attempts"]
+    assert n_att.min() > 0 and n_att.max() < sc["max_attempts"]
     assert np.mean(_sub(n_att, idx) == ref["n_attempt"]) >= 0.995
+    img = _np(out["image"])
+    assert np.all(np.isfinite(img)) and img.min() >= 0.0
+    fl = _np(out["flag"])
+    assert fl.min() >= 0 and fl.max() <= W.FLAG_MAXSTEP
 
 
 # ------------------------------------------------------------------------- transfer scheme E' (RK components)
@@ -310,7 +339,7 @@ def test_mixed_fp32_transfer_variant_accuracy_against_the_oracle(ody, orc, nu):
     out = ody.render_image(w["scene"], w["model"], nu, precision=ody.PREC_MIXED_FP32); _sync()
     ref = orc.render_image(w["scene"], w["model"], nu)
     assert np.array_equal(_np(out["flag"]).ravel(), ref["flag"])
-    assert np.array_equal(_np(out["n_attempt"]).ravel() == ref["n_attempt"], _np(out["n_attempt"]).ravel() == ref["n_attempt"])
+    assert np.mean(_np(out["n_attempt"]).ravel() == ref["n_attempt"]) >= 0.995       # the geodesic part is the FP64 one
     _check_image(_np(out["image"]).ravel(), ref["image"], f"mixed FP32 variant at {nu:g} Hz")
     # and it really is a different arithmetic: not bit-identical to the FP64 kernel
     base = ody.render_image(w["scene"], w["model"], nu); _sync()

@@ -255,23 +255,28 @@ def test_coordinate_time_output_matches_the_oracle(ody, orc, a, incl):
     assert np.array_equal(host["t"], gpu["t"])
 
 
-@pytest.mark.parametrize("a, incl", [(0.9, 2.0), (0.9, 178.0), (0.9999, 0.1), (0.0, 0.05)])
-def test_near_polar_observers_within_the_conditioning_limit(ody, orc, a, incl):
-    # Boyer-Lindquist coordinates are singular on the axis: rays of a near-polar observer have small L_z and turn
-    # at sin(theta_min) ~ |L_z| / b, where rounding differences are amplified by ~1 / sin(theta_min).
-    # Flags and step counts still agree; positions agree to 1e-6 instead of 1e-8, most of them far better.
+@pytest.mark.parametrize("a, incl, tol", [(0.9, 2.0, RTOL_STATE), (0.9, 178.0, RTOL_STATE), (0.5, 1.0, RTOL_STATE), (0.99, 4.0, RTOL_STATE),
+                                          (0.9999, 0.1, 1e-7), (0.0, 0.05, 1e-7)])
+def test_near_polar_observers(ody, orc, a, incl, tol):
+    # Boyer-Lindquist coordinates are singular on the axis (PAPER.md:L90 clamps sin(theta) for that reason).  Down to
+    # 1 degree from the pole the north_star tolerance of 1e-8 holds as everywhere else.  For observers 0.1 and 0.05
+    # degrees from the axis L_z is ~1e-3 of the impact parameter and the rays turn at sin(theta) ~ 1e-3: there the
+    # PROBLEM amplifies a relative perturbation of 1e-16 of the input to 1.4e-9 of the end state (measured on the
+    # oracle alone: tests/test_oracle_geodesics.py::test_conditioning_of_rays_of_a_nearly_polar_observer), so the
+    # rounding differences of ~900 steps may add up to a few 1e-8 (measured: 1.8e-8, three pixels above 1e-8);
+    # 1e-7 is allowed for these two scenes only.  Flags and step counts agree in all of them.
     sc = W.scene(a, incl, 48, 12.0, ny=40)
     out = ody.trace_geodesics(sc); _sync()
     gpu = {k: _np(v).ravel() for k, v in out.items()}
     ref = orc.trace_geodesics(sc)
     assert np.array_equal(gpu["flag"], ref["flag"])
-    assert np.mean(gpu["n_attempt"] == ref["n_attempt"]) >= 0.97
+    assert np.mean(gpu["n_attempt"] == ref["n_attempt"]) >= 0.995
     errs = []
     for k, k2 in (("r", "r"), ("theta", "th"), ("phi", "ph")):
         e = np.abs(gpu[k] - ref[k2]) / np.maximum(np.abs(ref[k2]), 1.0)
-        assert e.max() <= 1e-6, (k, e.max())
+        assert e.max() <= tol, (k, e.max())
         errs.append(e)
-    assert np.median(np.maximum.reduce(errs)) <= 1e-10
+    assert np.median(np.maximum.reduce(errs)) <= 1e-11
 
 
 def test_maximum_image_size_two_to_the_thirty_pixels(ody, orc):
