@@ -22,9 +22,22 @@ def _stale():
     return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
 
 
+def build_variant(out_path, extra_flags):
+    """Compile a variant of the library (e.g. ["-DODY_DEVICE_CHECKS"]) to out_path; returns out_path."""
+    nvcc = os.environ.get("NVCC", "nvcc")
+    cmd = [nvcc] + [f for f in NVCC_FLAGS if f not in ("-Xptxas", "-v")] + list(extra_flags) + ["-o", out_path] + SOURCES
+    res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed building " + out_path + "\n" + res.stderr[-2000:])
+    return out_path
+
+
 def build(force=False, verbose=False):
     """Compile if any source is newer than the library.  Returns the library path; the ptxas
-    resource report (registers, spills) is written next to it as libodyssey.ptxas.txt."""
+    resource report (registers, spills) is written next to it as libodyssey.ptxas.txt.
+    ODYSSEY_LIB in the environment names an already built library to load instead (a variant from build_variant)."""
+    if os.environ.get("ODYSSEY_LIB"):
+        return os.environ["ODYSSEY_LIB"]
     if not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")

@@ -33,6 +33,16 @@
 #include "geodesic.cuh"
 #include "emission.cuh"
 
+// -DODY_DEVICE_CHECKS builds the kernels with device-side assertions on every index into the stash, the transfer ring and
+// the output arrays (tests/test_gpu_device_checks.py builds that variant and runs the small configurations through it;
+// compute-sanitizer is not available on the B200 pool this was developed on).
+#ifdef ODY_DEVICE_CHECKS
+#include <cassert>
+#define ODY_CHECK(cond) assert(cond)
+#else
+#define ODY_CHECK(cond) ((void)0)
+#endif
+
 namespace ody {
 
 constexpr int M_NORMAL = 0, M_EQ = 1, M_CAP = 2, M_ESC = 3, M_FRESH = 4;       // lane modes
@@ -155,6 +165,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         int3 meta = make_int3(0, 0, 0);
         if (have) { er = FD(0, slot); esn = FD(1, slot); ecn = FD(2, slot); epr = FD(3, slot); eh = FD(4, slot); meta = make_int3(sm_ringi[slot], sm_ringi[FIFO_CAP + slot], sm_ringi[2 * FIFO_CAP + slot]); }
         const int o = (meta.y >> FIFO_ACC_BITS) & 31;
+        ODY_CHECK(cnt > 0 && cnt <= FIFO_CAP);
         double a1 = 0.0, e1 = 0.0;
         if (have) {
             RtPoint pt; rt_point<false, PREC>(P, sm_L[(threadIdx.x & ~31) + o], er, esn, ecn, epr, pt);
@@ -163,6 +174,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         }
         __syncwarp();
         const int pd = (int)((unsigned)meta.z - f_head);             // >= 0: the owner's previous point is in this batch, pd lanes up
+        ODY_CHECK(!have || pd < lane);
         double* const st = sm_rtw + o;                                // the owner's tau, T, I, a0, e0
         double dtau = 0.0, em = 0.0, phi = 1.0, w = 0.0;
         if (have) {
@@ -196,6 +208,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     auto fifo_finalize = [&]() {
         if (B.draining && (int)(f_head - (unsigned)LN(Q_LAST)) > 0) {
             int oflag = LN(Q_END), oatt = n_att, oacc = n_acc;
+            ODY_CHECK(pix >= 0 && pix < P.nx * P.ny && oflag >= 0 && oflag <= F_MAXSTEP);
             if (LN(Q_OATT) >= 0) { oflag = F_OPAQUE; oatt = LN(Q_OATT); oacc = LN(Q_OACC); }
             if (O.flag) O.flag[pix] = oflag;
             if (O.n_attempt) O.n_attempt[pix] = oatt;
@@ -235,6 +248,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                     State y0; double L0;
                     init_ray(P, x, yy, y0, L0);
                     const int idx = __popc(vm & ((1u << lane) - 1u));
+                    ODY_CHECK(idx >= 0 && idx < 32 && j * P.nx + i < P.nx * P.ny);
                     stash[idx] = y0.r; stash[32 + idx] = y0.th; stash[64 + idx] = y0.ph; stash[96 + idx] = y0.pr;
                     stash[128 + idx] = y0.pth; stash[160 + idx] = L0; stash[192 + idx] = __longlong_as_double((long long)(j * P.nx + i));
                 }
@@ -244,6 +258,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             const int rank = __popc(need & ((1u << lane) - 1u));
             const int st_cnt = st_w & 63;
             if (want && rank < st_cnt) {
+                ODY_CHECK(st_cnt <= 32 && st_cnt - 1 - rank >= 0);
                 const double* st = stash + (st_cnt - 1 - rank);
                 y.r = __ldcg(st); y.th = __ldcg(st + 32); y.ph = __ldcg(st + 64);
                 y.pr = __ldcg(st + 96); y.pth = __ldcg(st + 128); L = __ldcg(st + 160);
@@ -433,6 +448,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                 LN(Q_LAST) = (int)pos; B.prev_out = !inside;
             }
             f_tail += __popc(pm);
+            ODY_CHECK((int)(f_tail - f_head) >= 0 && (int)(f_tail - f_head) <= FIFO_CAP);
             __syncwarp();
             if ((int)(f_tail - f_head) >= 32 || ((drain_wait >= 2 || !any_active) && f_tail != f_head)) { fifo_process(); drain_wait = 0; }
         } else if (KIND == 2 && (commit || fresh)) {
@@ -487,6 +503,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             fifo_finalize();
             drain_wait = __any_sync(FULL, B.draining) ? drain_wait + 1 : 0;
         } else if (flag >= 0) {
+            ODY_CHECK(pix >= 0 && pix < P.nx * P.ny);
             if (O.flag) O.flag[pix] = flag;
             if (O.r) O.r[pix] = y.r;
             if (O.th) O.th[pix] = y.th;
