@@ -20,6 +20,7 @@ reference is a paper).
 """
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -246,6 +247,18 @@ def time_extra_configs(ody, torch):
                                   frequencies=len(w3["nu"]))
     m_rk = dict(w2["model"], rt_scheme=W.RT_RK_COMPONENTS)
     res["C2 rt_scheme=RK components"] = timed(lambda: ody.render_image(w2["scene"], m_rk, w2["nu"][0]), w2["scene"]["nx"] * w2["scene"]["ny"])
+    w8 = W.C3(n=1024, nf=8)
+    res["C3 flow, 1024^2 x 8 frequencies (fused spectrum kernel)"] = dict(
+        timed(lambda: ody.render_spectrum(w8["scene"], w8["model"], w8["nu"]), 1024 * 1024), frequencies=8)
+    w32 = W.C3(n=1024)
+    res["C3 flow, 1024^2 x 32 frequencies (two-phase path in bands)"] = dict(
+        timed(lambda: ody.render_spectrum(w32["scene"], w32["model"], w32["nu"]), 1024 * 1024), frequencies=32)
+    ody.trim_scratch(0)
+    hs_scene, hs_model = W.scene(0.0, 60.0, 512, 12.0), W.model_hot_spot()
+    t_obs = [k * 2.0 * math.pi * (6.0 ** 1.5) / 32 for k in range(32)]
+    res["hot spot a=0 i=60 512^2, 32 phases"] = dict(timed(lambda: ody.render_hotspot(hs_scene, hs_model, t_obs), 512 * 512), phases=32)
+    tab1 = W.scene(0.95, 60.0, 1024, 10.0)
+    res["paper Table 1 set-up: geodesics only a=0.95 i=60 1024^2"] = timed(lambda: ody.trace_geodesics(tab1), 1024 * 1024)
     for a in (0.0, 0.5, 0.9, 0.998):
         for n in (1024, 2048, 4096):
             w4 = W.C4(n=n, a=a)

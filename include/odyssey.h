@@ -28,7 +28,7 @@
  *   - Scratch: every launch takes what it needs — its work-queue counter, one stash of 32 prepared rays per
  *     warp of the grid (~5 MB in all, whatever the image size), in spectrum mode the per-frequency accumulators
  *     or node lists described there — from a stream-ordered memory pool of the library's own (created lazily per
- *     device, cudaMallocFromPoolAsync / cudaFreeAsync on `cuda_stream`; cached blocks above 6 GiB go back to the
+ *     device, cudaMallocFromPoolAsync / cudaFreeAsync on `cuda_stream`; cached blocks above 12 GiB go back to the
  *     driver at the next synchronisation; odyssey_trim_scratch() returns more, odyssey_shutdown() everything).
  *     Nothing is shared between launches, so any number of calls may be in flight on any number of streams.
  *   - One kernel launch of this library per call (the persistent integrator builds the initial conditions of its

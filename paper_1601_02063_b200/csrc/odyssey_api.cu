@@ -72,7 +72,9 @@ int device_state(DevState** out, int* dev_out) {
         props.location.type = cudaMemLocationTypeDevice;
         props.location.id = dev;
         CUDA_TRY(cudaMemPoolCreate(&D.pool, &props));
-        unsigned long long keep = 6ull << 30;      // cached scratch above 6 GiB goes back to the driver at the next synchronisation
+        // cached scratch above 12 GiB goes back to the driver at the next synchronisation (a band of the two-phase spectrum
+        // path holds ~10 GB of node lists and synchronises once per band: a lower threshold would re-allocate them every band)
+        unsigned long long keep = 12ull << 30;
         CUDA_TRY(cudaMemPoolSetAttribute(D.pool, cudaMemPoolAttrReleaseThreshold, &keep));
         D.ready = true;
     }
@@ -239,7 +241,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
 #endif
 constexpr int NT_MAIN = 128, MINB_MAIN = ODY_MINB_MAIN;     // 96 registers per thread at most
 constexpr int MINB_SPOT = 4;                    // thin disk, hot spot, Novikov-Thorne disk and the coordinate-time variant: 4 blocks per SM keep them free of spills
-constexpr int MINB_RK = 2;                      // transfer scheme E' (RK components): the in-loop transfer code wants > 168 registers
+constexpr int MINB_RK = 4;                      // transfer scheme E' (RK components)
 constexpr int NT_SPEC = 128, MINB_SPEC = 3;     // 168 registers (the unrolled frequency loop wants them); per-frequency accumulators in a global scratch buffer
 
 typedef void (*KernelFn)(const Params, const Outputs);
@@ -273,6 +275,7 @@ size_t smem_bytes(int kind, bool spec, int nf, int nbins, int rts = 0) {
     if (kind == 1) return stages + (size_t)(nbins > 0 ? nbins : 1) * sizeof(double);
     if (kind == 4) return stages + (size_t)MAX_FREQ * sizeof(double);
     if (uses_fifo(kind, spec, rts)) return stages + (size_t)fifo_doubles_per_block(NT_MAIN) * sizeof(double);
+    if (kind == 2 && rts == 1) return stages + (size_t)20 * NT_MAIN * sizeof(double);      // scheme E': the stage states
     return stages;
 }
 

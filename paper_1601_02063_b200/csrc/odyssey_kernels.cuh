@@ -118,6 +118,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
     double* const sm_hnext = sm_red + NT + (NT / 32) * FIFO_DOUBLES + 3 * NT;             // [2][NT]: next step length, φ slope of the first stage
     constexpr int Q_OATT = 0, Q_OACC = 1, Q_LAST = 2, Q_END = 3, Q_PIX = 4, Q_NACC = 5;                          // opaque crossing: n_attempt (-1: none), n_accept; latest ring position; end flag
     double* const sm_rtw = smem + (smem_per_thread(RTS) - 5) * NT + (threadIdx.x & ~31);  // RT state of this warp's lane 0
+    double* const sm_ss = sm_red + threadIdx.x;                                           // (RTS == 1) [4][5][NT]: r, sinθ, cosθ, p_r of the stage states
+#define SS(c, st) sm_ss[((c) * 5 + (st) - 1) * NT]
 #define FD(f, slot) sm_ring[(f) * FIFO_CAP + (slot)]
 #define LN(q) sm_lane[(q) * NT + threadIdx.x]
     unsigned f_head = 0, f_tail = 0;                                                      // ring positions (warp-uniform)
@@ -303,14 +305,6 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
         double ph5 = kRkB5[TAB][0] * kph0;
         double phe = kRkBE[TAB][0] * kph0;
         double t5 = TIME ? kRkB5[TAB][0] * kt0 : 0.0;
-        // scheme E': running fifth-order sums of a and of eps exp(-tau) over the stages; stage 0 = cached start values
-        double rk_tau = 0.0, rk_I = 0.0, tau_n = 0.0;
-        if (RTS == 1) {
-            tau_n = RT1(0);
-            rk_tau = kRkB5[TAB][0] * RT1(3);
-            rk_I = kRkB5[TAB][0] * RT1(4) * d_exp_lo(-tau_n);
-            K.set(4, 0, RT1(3));
-        }
         // One attempt is ONE straight-line block: the five stage evaluations, the fifth-order result, the error
         // norm, the controller and the evaluation of f at the trial end state run for EVERY lane of the warp, and
         // only the bookkeeping that follows is predicated.  A lane without a running attempt (fresh, idle) computes
@@ -327,13 +321,8 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             stage_point<TAB, I>(K, y, h_try, ir, ith, ipr, ipth);                                              \
             geodesic_rhs<TIME != 0>(a, a2, L, ir, ith, ipr, ipth, k, sn, cn);                                  \
             if (TIME) t5 = fma(kRkB5[TAB][I], k.t, t5);                                                        \
-            if (RTS == 1) {                                      /* coefficients at this stage state */       \
-                RtPoint pt; rt_point<false>(P, L, ir, sn, cn, ipr, pt);                                        \
-                double as, es; rt_coefficients<false>(P, pt, freq_of(P, 0), as, es);                           \
-                const double ts = stage_sum<TAB, I>(K, 4);                                                     \
-                rk_tau = fma(kRkB5[TAB][I], as, rk_tau);                                                       \
-                rk_I = fma(kRkB5[TAB][I] * es, d_exp_lo(-fma(h_try, ts, tau_n)), rk_I);                        \
-                if (I < STAGE_SLOTS) K.set(4, I, as);                                                          \
+            if (RTS == 1) {                /* scheme E': where this stage was (its coefficients are formed on acceptance) */ \
+                SS(0, I) = ir; SS(1, I) = sn; SS(2, I) = cn; SS(3, I) = ipr;                                   \
             }                                                                                                  \
             store_stage<TAB, I>(K, k, ph5, phe);                                                               \
         }
@@ -470,7 +459,24 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
             } else {
                 double a1, e1; rt_coefficients<false, PREC>(P, pt, freq_of(P, 0), a1, e1);
                 if (commit && RTS == 1) {
-                    double tau = RT1(0);
+                    // Scheme E': tau and I as two more Runge-Kutta components.  The coefficients at the five stage
+                    // states of the step just ACCEPTED (a rejected attempt needs none) in ONE rolled loop around one
+                    // copy of the coefficient code; stage 0 = the values cached at the step's start.
+                    const double tau_n = RT1(0);
+                    double rk_tau = kRkB5[TAB][0] * RT1(3);
+                    double rk_I = kRkB5[TAB][0] * RT1(4) * d_exp_lo(-tau_n);
+                    K.set(4, 0, RT1(3));
+#pragma unroll 1
+                    for (int st = 1; st <= 5; ++st) {
+                        RtPoint ps; rt_point<false>(P, L, SS(0, st), SS(1, st), SS(2, st), SS(3, st), ps);
+                        double as, es; rt_coefficients<false>(P, ps, freq_of(P, 0), as, es);
+                        double ts = 0.0;
+                        for (int j = 0; j < st; ++j) ts = fma(kRkA[TAB][st][j], K.get(4, j), ts);
+                        rk_tau = fma(kRkB5[TAB][st], as, rk_tau);
+                        rk_I = fma(kRkB5[TAB][st] * es, d_exp_lo(-fma(h_try, ts, tau_n)), rk_I);
+                        if (st < STAGE_SLOTS) K.set(4, st, as);
+                    }
+                    double tau = tau_n;
                     if (!(tau > P.tau_max)) {                              // frozen once tau > tau_max
                         RT1(2) = fma(h_try, rk_I, RT1(2));
                         tau = fma(h_try, rk_tau, tau);
@@ -592,6 +598,7 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
 #undef RT1
 #undef FD
 #undef LN
+#undef SS
     // ---------------------------------------------------------------------- block-level reductions
     if ((SPEC || KIND == 4) && O.nuLnu) {
         __syncthreads();
