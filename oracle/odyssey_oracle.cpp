@@ -444,7 +444,15 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
     const Tableau T = make_tableau(S.tableau);
     const Flow F = make_flow(S.a);
     const double r_cap = horizon_radius(S.a) + S.horizon_eps;
-    const double r_in = (M.r_in > 0.0) ? M.r_in : F.r_isco;
+    double r_in = (M.r_in > 0.0) ? M.r_in : F.r_isco;
+    if (M.kind == 3 && !(M.r_in > 0.0)) {
+        // [reading HS] PAPER.md:L259 lights everything "within d < 4 r_spot" of a centre that orbits AT r_isco, so the
+        // opaque plane must reach inwards to the inner edge of the spot (d is measured in the pseudo-Cartesian radius
+        // sqrt(r^2 + a^2) of eqs. (33), (34)); with the thin disk's default (r_isco) the inner half would never be lit.
+        const double rs = (M.spot_r_orbit > 0.0) ? M.spot_r_orbit : F.r_isco;
+        const double Rin = std::sqrt(rs * rs + S.a * S.a) - 4.0 * M.spot_size;
+        r_in = (Rin > std::fabs(S.a)) ? std::sqrt(Rin * Rin - S.a * S.a) : 0.0;
+    }
     double h = S.h0;
     int n_attempt = 0, n_accept = 0, flag = -1;
     bool on_equator = false;

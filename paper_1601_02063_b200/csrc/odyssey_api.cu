@@ -129,7 +129,7 @@ int check_model(const odyssey_model* M) {
     if (M->kind < ODYSSEY_KIND_NONE || M->kind > ODYSSEY_KIND_NT_DISK) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "unknown model kind %d", M->kind);
     if (M->kind == ODYSSEY_KIND_HOT_SPOT) {
         if (!(M->spot_size > 0.0)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spot_size = %g must be > 0", M->spot_size);
-        if (M->spot_r_orbit > 0.0 && !(M->spot_r_orbit > 1.0 + std::sqrt(1.0)))
+        if (M->spot_r_orbit > 0.0 && !(M->spot_r_orbit > 1.0))
             return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spot_r_orbit = %g must lie outside the horizon (or be <= 0 for r_isco)", M->spot_r_orbit);
     }
     if (M->kind == ODYSSEY_KIND_THIN_DISK || M->kind == ODYSSEY_KIND_HOT_SPOT) {
@@ -214,6 +214,12 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
     }
     if (M->kind == ODYSSEY_KIND_THIN_DISK || M->kind == ODYSSEY_KIND_HOT_SPOT) {
         P->r_in = (M->r_in > 0.0) ? M->r_in : P->r_isco;
+        if (M->kind == ODYSSEY_KIND_HOT_SPOT && !(M->r_in > 0.0)) {
+            // reading HS: the plane is opaque (and lit) down to the inner edge of the spot, 4 r_spot inside its centre
+            // in the pseudo-Cartesian radius of eqs. (33), (34), so that the whole Gaussian of PAPER.md:L259 is seen
+            const double R_in = P->spot_R - 4.0 * M->spot_size;
+            P->r_in = (R_in > std::fabs(S.a)) ? std::sqrt(R_in * R_in - S.a * S.a) : 0.0;
+        }
         P->r_out = M->r_out; P->emis_index = M->emis_index; P->g_power = M->g_power;
         P->g_lo = M->g_lo; P->g_hi = M->g_hi; P->nbins = M->nbins;
     }
@@ -610,6 +616,8 @@ int odyssey_render_hotspot(const odyssey_scene* scene, const odyssey_model* mode
     rc = check_model(model);
     if (rc) return rc;
     if (model->kind != ODYSSEY_KIND_HOT_SPOT) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "hot-spot mode needs model kind 3, got %d", model->kind);
+    if (model->spot_r_orbit > 0.0 && !(model->spot_r_orbit > 1.0 + std::sqrt(1.0 - scene->a * scene->a)))
+        return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "spot_r_orbit = %g lies inside the horizon of a = %g", model->spot_r_orbit, scene->a);
     if (nt < 1 || nt > ODYSSEY_MAX_FREQ) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "nt = %d outside [1, %d]", nt, ODYSSEY_MAX_FREQ);
     if (!t_obs_host) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "t_obs_host is NULL");
     for (int k = 0; k < nt; ++k)

@@ -40,7 +40,11 @@ def test_pixel_values_follow_eq36_at_the_retarded_spot_position():
 def test_geometry_of_the_crossing_is_the_thin_disk_one():
     sc = W.scene(0.9, 60.0, 40, 12.0)
     hs = O.render_hotspot(sc, W.model_hot_spot(), [0.0])
-    td = O.render_image(sc, W.model_thin_disk())
+    # the hot-spot plane reaches inwards to the inner edge of the spot: R_in = sqrt(r_s^2 + a^2) - 4 r_spot (reading HS)
+    kc = O.kerr_constants(0.9)
+    R_in = math.sqrt(kc["r_isco"] ** 2 + 0.81) - 4 * 0.5
+    assert R_in < 0.9                                              # here the inner edge lies inside the hole: the plane is lit down to the capture radius
+    td = O.render_image(sc, W.model_thin_disk(r_in=1e-9))
     assert np.array_equal(hs["flag"], td["flag"])
     assert np.array_equal(hs["g"], td["aux0"]) and np.array_equal(hs["r_e"], td["aux1"])
 
@@ -100,3 +104,18 @@ def test_flux_peaks_when_the_approaching_spot_is_seen():
     kmax, kmin = int(np.argmax(o["lightcurve"])), int(np.argmin(o["lightcurve"]))
     gw = lambda k: (o["images"][k] * o["g"]).sum() / o["images"][k].sum()
     assert gw(kmax) > 1.0 > gw(kmin)
+
+
+def test_lit_region_is_the_whole_gaussian_symmetric_about_the_orbit():
+    """everything within d < 4 r_spot of the centre is lit, and the centre orbits AT r_isco — so the lit
+    region must extend as far inside the orbit as outside it (with the thin disk's inner edge r_isco as the plane's
+    edge the inner half of the spot would be dark).  Seen nearly face-on, a = 0: lit crossings span r_s - 2 .. r_s + 2."""
+    sc = W.scene(0.0, 0.5, 160, 10.0)
+    mo = W.model_hot_spot(r_spot=0.5)
+    out = O.render_hotspot(sc, mo, [0.0])
+    lit = out["images"][0] > 0
+    assert lit.sum() > 100
+    re = out["r_e"][lit]
+    assert re.min() == pytest.approx(6.0 - 2.0, abs=0.15) and re.max() == pytest.approx(6.0 + 2.0, abs=0.15)
+    # and the brightest pixel sits at the centre of the spot, not at the plane's edge
+    assert out["r_e"][np.argmax(out["images"][0])] == pytest.approx(6.0, abs=0.15)
