@@ -486,7 +486,10 @@ void trace_ray(const Scene& S, const Model& M, int nf, const double* nu, double 
                 if (std::fabs(f) <= ftol) break;
                 double dy[NV];
                 rhs(ray, ynew, dy);
-                h_used -= f / dy[comp];
+                // safeguard [reading J]: the Newton update must stay inside (0, ~the accepted step] (h_next >= 0.9 h);
+                // a flat or non-finite slope, or a non-finite trial state, halves the step length instead
+                double hn = h_used - f / dy[comp];
+                h_used = (hn > 0.0 && hn <= 1.2 * h_next) ? hn : 0.5 * h_used;
                 rk_attempt(ray, T, y, h_used, ynew, yerr, ystage);
                 ++n_attempt;
             }

@@ -112,6 +112,8 @@ int check_scene(const odyssey_scene* S) {
     if (!(S->r_obs > 0.0) || !(S->h0 > 0.0) || !(S->r_esc > 0.0) || !(S->horizon_eps >= 0.0) || S->max_attempts <= 0)
         return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "r_obs, h0, r_esc, max_attempts must be positive and horizon_eps >= 0");
     if (S->max_attempts >= (1 << FIFO_ACC_BITS)) return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "max_attempts = %d must be below 2^%d", S->max_attempts, FIFO_ACC_BITS);
+    if (!(std::fabs(std::sin(S->theta_obs)) > 1e-10))
+        return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "observer on the spin axis (theta_obs = %g): the Boyer-Lindquist azimuth of the ray through the image centre is undefined; tilt by >= 1e-9 rad", S->theta_obs);
     if (!(S->x_max > S->x_min) || !(S->y_max > S->y_min))
         return fail(ODYSSEY_ERR_INVALID_ARGUMENT, "image-plane extent is empty");
     {   // every ray must come back out through r = r_esc: a ray whose impact parameter exceeds r_esc turns around

@@ -373,8 +373,11 @@ odyssey_kernel(const __grid_constant__ Params P, const __grid_constant__ Outputs
                                                      : ((mode == M_CAP) ? P.r_cap : P.r_esc);
                 const double f = ((mode == M_EQ) ? yn.th : yn.r) - target;
                 const double ftol = 1e-12 * fmax(1.0, fabs(target));
-                if (loc_it < LOCATE_MAX && fabs(f) > ftol) {           // Newton on the step size, re-take from y
-                    h_try -= f / ((mode == M_EQ) ? kn.th : kn.r);
+                if (loc_it < LOCATE_MAX && !(fabs(f) <= ftol)) {       // Newton on the step size, re-take from y
+                    // safeguard (reading J): a flat or non-finite slope, or a non-finite trial state, must not throw the step
+                    // length out of (0, ~the accepted step] (h_next >= 0.9 x the accepted step): halve instead
+                    const double hn = h_try - f / ((mode == M_EQ) ? kn.th : kn.r);
+                    h_try = (hn > 0.0 && hn <= 1.2 * h_next) ? hn : 0.5 * h_try;
                     retake = true;
                     break;
                 }
