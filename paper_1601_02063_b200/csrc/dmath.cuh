@@ -13,8 +13,8 @@
 //   d_exp, d_expm1         : x = k ln2 + r, e^r = 1 + r q(r), scaling through the exponent field
 //   d_log                  : x = 2^e m, m in [sqrt(1/2), sqrt(2)), log m = 2 atanh((m-1)/(m+1))
 //
-// Accuracy: a few ulp (tests/test_dmath.py compares against libm on the host build of this header and
-// tests/test_gpu_dmath.py on the device).  Polynomial tables: dmath_coeffs.h (gen_dmath_coeffs.py).
+// Accuracy: a few ulp (tests/test_dmath.py: the host build of this header against libm, and the device build
+// through odyssey_eval_math against libm and scipy).  Polynomial tables: dmath_coeffs.h (gen_dmath_coeffs.py).
 #pragma once
 #include <stdint.h>
 #include "dmath_coeffs.h"
