@@ -247,8 +247,11 @@ def time_extra_configs(ody, torch):
                                   frequencies=len(w3["nu"]))
     m_rk = dict(w2["model"], rt_scheme=W.RT_RK_COMPONENTS)
     res["C2 rt_scheme=RK components"] = timed(lambda: ody.render_image(w2["scene"], m_rk, w2["nu"][0]), w2["scene"]["nx"] * w2["scene"]["ny"])
+    w3f = W.C3(n=1024, nf=3)
+    res["C3 flow, 1024^2 x 3 frequencies (fused spectrum kernel)"] = dict(
+        timed(lambda: ody.render_spectrum(w3f["scene"], w3f["model"], w3f["nu"]), 1024 * 1024), frequencies=3)
     w8 = W.C3(n=1024, nf=8)
-    res["C3 flow, 1024^2 x 8 frequencies (fused spectrum kernel)"] = dict(
+    res["C3 flow, 1024^2 x 8 frequencies (two-phase path in bands)"] = dict(
         timed(lambda: ody.render_spectrum(w8["scene"], w8["model"], w8["nu"]), 1024 * 1024), frequencies=8)
     w32 = W.C3(n=1024)
     res["C3 flow, 1024^2 x 32 frequencies (two-phase path in bands)"] = dict(

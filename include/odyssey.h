@@ -144,7 +144,7 @@ int odyssey_render_image(const odyssey_scene* scene, const odyssey_model* model,
 /* nf <= 32 observed frequencies integrated simultaneously along each geodesic (kind 2 only;
  * BASELINE.json:configs[3]).  images[nf][ny][nx] = I_nu; nuLnu[nf] = 4π nu r_g^2 Δx Δy Σ_pixels I_nu
  * (erg/s; the distance cancels).  nu_hz_host is HOST memory.  rt_scheme must be ODYSSEY_RT_PER_STEP.
- * Two code paths, same results to rounding: images of up to ~1.5e5 rays, and larger images with nf >= 12, take a
+ * Two code paths, same results to rounding: images of up to ~1.5e5 rays, and larger images with nf >= 4, take a
  * two-phase path (record the geodesics once, then one lane per (ray, frequency); larger images band by band); it
  * synchronises `cuda_stream` ONCE per band inside the call to read an overflow flag, and uses stream-ordered scratch
  * (64 KB per ray of a band, ~10 GB at most).  Larger images with fewer frequencies take one fused kernel, no

@@ -335,7 +335,10 @@ Outputs no_outputs() { Outputs O; std::memset(&O, 0, sizeof(O)); return O; }
 // against 3.0 ms fused, for a fixed ~19 ms per megaray of recording).  Images larger than one band are processed
 // band by band (whole rows), so the node lists stay at ~10 GB whatever the image size.
 constexpr int TWO_PHASE_WAVES = 2;             // rays per band, in waves of the record kernel's resident lanes
-constexpr int TWO_PHASE_MIN_NF = 12;           // larger images with fewer frequencies take the fused kernel
+#ifndef ODY_TWO_PHASE_MIN_NF
+#define ODY_TWO_PHASE_MIN_NF 4
+#endif
+constexpr int TWO_PHASE_MIN_NF = ODY_TWO_PHASE_MIN_NF;   // larger images with fewer frequencies take the fused kernel (1024^2: 17.5 vs 21.1 ms at 2, 23.8 vs 23.6 at 4, 33.3 vs 29.4 at 8)           // larger images with fewer frequencies take the fused kernel
 constexpr long long NODE_CAP = 1024;           // nodes per ray of the first, fixed-capacity attempt (64 KB per ray)
 
 template <int G>
