@@ -250,7 +250,7 @@ void fill_params(const odyssey_scene& S, const odyssey_model* M, const double* n
 constexpr int NT_MAIN = 128, MINB_MAIN = ODY_MINB_MAIN;     // 96 registers per thread at most
 constexpr int MINB_SPOT = 4;                    // thin disk, hot spot, Novikov-Thorne disk and the coordinate-time variant: 4 blocks per SM keep them free of spills
 constexpr int MINB_RK = 4;                      // transfer scheme E' (RK components)
-constexpr int NT_SPEC = 128, MINB_SPEC = 3;     // 168 registers (the unrolled frequency loop wants them); per-frequency accumulators in a global scratch buffer
+constexpr int NT_SPEC = 128, MINB_SPEC = 4;     // 126 registers, no spills; per-frequency accumulators in a global scratch buffer
 
 typedef void (*KernelFn)(const Params, const Outputs);
 
