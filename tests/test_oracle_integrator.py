@@ -120,3 +120,37 @@ def test_step_controller_accept_reject_statistics():
     assert np.all(lo["n_attempt"] - lo["n_accept"] < 0.5 * lo["n_attempt"])
     ratio = hi["n_accept"].sum() / lo["n_accept"].sum()
     assert 1.8 < ratio < 3.2, ratio          # 100^(1/5) = 2.51
+
+
+def test_step_sequence_is_that_of_press_et_als_controller():
+    """PAPER.md:L90 cites Press et al. (1992) for the step control; their driver (rkqs) uses SAFETY 0.9, PGROW -0.2,
+    PSHRNK -0.25, ERRCON 1.89e-4 (growth at most x 5) and shrinks by at most x 10 (reading G).  The oracle's accepted
+    step lengths are re-derived here from those numbers, with the oracle's embedded pair and error norm as black boxes:
+    starting from h0, every trial step is accepted iff err <= 1, h <- h min(5, 0.9 err^-0.2) after an accepted step and
+    h <- h max(0.1, 0.9 err^-0.25) after a rejected one.  Swapping the two exponents, or another safety factor,
+    changes the sequence at its first rejection and fails the comparison (checked for the swap below)."""
+    sc = W.scene(0.9, 60.0, 64, 10.0, rtol=1e-8)
+    a = sc["a"]
+    for x, y in [(-6.0, 2.0), (7.0, -1.0)]:
+        nodes, cons, res = O.trace_path(sc, W.model_none(), x, y)
+        st, _ = O.init_ray(sc, x, y)
+        h_acc = np.diff(nodes[:, 5])                                    # accepted step lengths (node 0 is the start; the last step is event-located)
+
+        def simulate(pgrow, pshrnk, n_steps):
+            yv, h, out, attempts = np.array(st[:5], float), sc["h0"], [], 0
+            while len(out) < n_steps:
+                ynew, yerr = O.rk_attempt(a, cons["E"], cons["L"], sc["tableau"], yv, h)
+                err = O.error_norm(yv, yerr, sc["rtol"])
+                attempts += 1
+                if err <= 1.0:
+                    out.append(h); yv = ynew
+                    h *= 5.0 if err < 1.89e-4 else min(5.0, 0.9 * err ** pgrow)
+                else:
+                    h *= max(0.1, 0.9 * err ** pshrnk)
+            return np.array(out), attempts
+        n = len(h_acc) - 1                                              # all but the located last step
+        sim, attempts = simulate(-0.2, -0.25, n)
+        assert res["n_attempt"] > res["n_accept"]                       # the ray does have rejected attempts
+        assert np.allclose(sim, h_acc[:n], rtol=1e-12, atol=0.0)
+        swapped, _ = simulate(-0.25, -0.2, n)
+        assert not np.allclose(swapped, h_acc[:n], rtol=1e-6, atol=0.0)
