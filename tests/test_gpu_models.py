@@ -313,6 +313,11 @@ def test_banded_two_phase_spectrum_on_a_large_image_matches_the_oracle_and_the_o
     ("small emitting region", dict(a=0.998, incl=85.0), dict(r_rt_out=12.0), 230e9),
     ("face-on", dict(a=0.7, incl=0.5), dict(), 230e9),
     ("loose tolerance", dict(a=0.9375, incl=30.0, rtol=1e-5), dict(), 230e9),
+    ("tiny tau_max: nearly every ray ends OPAQUE after a few emitting steps (the ring's run-ahead is discarded)", dict(a=0.9375, incl=30.0), dict(tau_max=1e-7), 230e9),
+    ("negative tau_max: OPAQUE at the first accepted step", dict(a=0.5, incl=60.0), dict(tau_max=-1.0), 230e9),
+    ("few attempts allowed: rays end MAXSTEP with points still in the ring", dict(a=0.9, incl=60.0, max_attempts=120), dict(), 230e9),
+    ("observer inside a bright, outward-weighted medium: the start point's coefficients matter", dict(a=0.9375, incl=30.0, r_obs=100.0),
+     dict(n0=1e3, n_index=1.0, T0=3e10, T_index=0.0, h_over_r=10.0), 230e9),
 ])
 def test_riaf_parameter_sweep_matches_the_oracle(ody, orc, label, scene_kw, model_kw, nu):
     kw = dict(scene_kw)
@@ -322,6 +327,9 @@ def test_riaf_parameter_sweep_matches_the_oracle(ody, orc, label, scene_kw, mode
     ref = orc.render_image(sc, mo, nu)
     assert np.array_equal(_np(out["flag"]).ravel(), ref["flag"]), label
     assert np.mean(_np(out["n_attempt"]).ravel() == ref["n_attempt"]) >= 0.99, label
+    assert np.mean(_np(out["n_accept"]).ravel() == ref["n_accept"]) >= 0.99, label
+    tau, tau_ref = _np(out["aux0"]).ravel(), ref["aux0"]
+    assert np.allclose(tau, tau_ref, rtol=1e-6, atol=1e-300), label
     img = _np(out["image"]).ravel()
     if ref["image"].max() == 0.0:
         assert np.all(img == 0.0), label
@@ -329,6 +337,8 @@ def test_riaf_parameter_sweep_matches_the_oracle(ody, orc, label, scene_kw, mode
         _check_image(img, ref["image"], label)
     if "OPAQUE" in label:
         assert np.mean(ref["flag"] == W.FLAG_OPAQUE) > 0.3
+    if "MAXSTEP" in label:
+        assert np.mean(ref["flag"] == W.FLAG_MAXSTEP) > 0.1
 
 
 # ------------------------------------------------------------- mixed-precision transfer variant (north_star (c))
