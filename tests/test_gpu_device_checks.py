@@ -68,3 +68,36 @@ def test_guard_bands_around_the_output_arrays_stay_untouched(ody, nx, ny):
             inside[pad + k * (n + pad): pad + k * (n + pad) + n] = True
         assert np.all(h[~inside] == -777), "a guard band was written"
         assert not np.any(h[inside] == -777), "an output element was not written"
+
+
+def test_transfer_ring_does_not_change_a_single_bit(ody):
+    """batching the transfer coefficients through the per-warp ring changes which lane evaluates a point and
+    when, not the arithmetic or its order per ray.  The library rebuilt without the ring (-DODY_RT_FIFO=0: every lane
+    evaluates its own point in the trip that produced it) must give the same image, optical depth, flags and step counts
+    bit for bit — thin and optically thick (most rays ending OPAQUE: the ring's run-ahead is discarded)."""
+    import torch
+    from paper_1601_02063_b200 import build as B
+    tmp = tempfile.mkdtemp(prefix="ody_nofifo_")
+    lib = os.path.join(tmp, "libodyssey_nofifo.so")
+    B.build_variant(lib, ["-DODY_RT_FIFO=0"])
+    code = r'''
+import sys
+sys.path.insert(0, %r)
+import numpy as np, torch, workloads as W
+import paper_1601_02063_b200 as ody
+w = W.C2(n=320)
+for tag, nu, kw in (("thin", 230e9, {}), ("thick", 5e9, {"tau_max": 0.5})):
+    out = ody.render_image(dict(w["scene"], ny=250), dict(w["model"], **kw), nu); torch.cuda.synchronize()
+    np.savez(%r + "/" + tag + ".npz", **{k: v.cpu().numpy() for k, v in out.items() if v is not None})
+print("DONE")
+''' % (ROOT, tmp)
+    res = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, env=dict(os.environ, ODYSSEY_LIB=lib), timeout=900)
+    assert res.returncode == 0 and "DONE" in res.stdout, res.stdout[-1000:] + res.stderr[-3000:]
+    w = W.C2(n=320)
+    for tag, nu, kw in (("thin", 230e9, {}), ("thick", 5e9, {"tau_max": 0.5})):
+        out = ody.render_image(dict(w["scene"], ny=250), dict(w["model"], **kw), nu); torch.cuda.synchronize()
+        ref = np.load(os.path.join(tmp, tag + ".npz"))
+        for k in ("image", "aux0", "flag", "n_attempt", "n_accept"):
+            assert np.array_equal(out[k].cpu().numpy(), ref[k]), (tag, k)
+        if tag == "thick":
+            assert np.mean(ref["flag"] == W.FLAG_OPAQUE) > 0.3
