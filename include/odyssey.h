@@ -20,7 +20,11 @@
  *     and returns without synchronising; the caller synchronises before reading.
  *   - HOST entry points (suffix _host): same arguments but every output pointer is HOST memory; the
  *     call allocates device scratch, runs the same kernels, copies the results back and returns
- *     after the copies have completed (synchronous).
+ *     after the copies have completed (synchronous).  odyssey_trace_geodesics_host and odyssey_render_image_host
+ *     render images of 2^21 pixels and more in up to 16 bands of whole rows that alternate between two streams
+ *     of the library's own, so that a band's device->host copies run under the next band's kernel (pinned host
+ *     buffers make the copies asynchronous; pageable ones still work); every pixel is bit-identical to the
+ *     DEVICE call's.  Concurrent _host calls from several host threads share those two streams.
  *   - The structs and the frequency list are always HOST memory, read during the call only.
  *   - Return value: ODYSSEY_OK (0) or a negative odyssey_status.  After a failure
  *     odyssey_last_error() returns a static, thread-local, NUL-terminated description.
